@@ -1,0 +1,152 @@
+"""ctypes wrapper of the float64 CPU oracle (oracle/mwax_oracle.c).
+
+TEST INFRASTRUCTURE ONLY: imported by tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs.  Nothing under paper_2303_11557_b200/ imports it, and it imports nothing from there.
+All arithmetic is in the C file; this module only marshals numpy arrays.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mwax_oracle.c")
+_LIB = os.path.join(_HERE, "libmwax_oracle.so")
+_lib = None
+
+AVG_CENTRE_SYMMETRIC = 0
+AVG_BLOCK = 1
+
+
+def build(force: bool = False) -> str:
+    """gcc -O2 (no fast-math) -fopenmp; building the checker is not using it."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", "-std=c99", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        dp = ctypes.POINTER(ctypes.c_double)
+        ip = ctypes.POINTER(ctypes.c_int)
+        i8p = ctypes.POINTER(ctypes.c_int8)
+        i32p = ctypes.POINTER(ctypes.c_int32)
+        lib.mwax_oracle_dft_naive.argtypes = [ctypes.c_int, dp, dp]
+        lib.mwax_oracle_fft.argtypes = [ctypes.c_int, dp, dp]
+        lib.mwax_oracle_weights.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp]
+        lib.mwax_oracle_spectra.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                            i8p, ctypes.c_int64, dp]
+        lib.mwax_oracle_correlate.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp]
+        lib.mwax_oracle_average.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp]
+        lib.mwax_oracle_fx.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                       ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp]
+        lib.mwax_oracle_xcorr_i8.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, i8p, i32p]
+        lib.mwax_oracle_threads.argtypes = []
+        _lib = lib
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed with code {rc}")
+
+
+def _sel(sel, n_inputs):
+    s = np.ascontiguousarray(np.arange(n_inputs) if sel is None else sel, dtype=np.int32)
+    return s, s.ctypes.data_as(ctypes.POINTER(ctypes.c_int))
+
+
+def threads() -> int:
+    return int(_load().mwax_oracle_threads())
+
+
+def dft_naive(x: np.ndarray) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    out = np.empty_like(x)
+    _check(_load().mwax_oracle_dft_naive(x.size, _dp(x.view(np.float64)), _dp(out.view(np.float64))), "dft_naive")
+    return out
+
+
+def fft(x: np.ndarray) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.complex128)
+    out = np.empty_like(x)
+    _check(_load().mwax_oracle_fft(x.size, _dp(x.view(np.float64)), _dp(out.view(np.float64))), "fft")
+    return out
+
+
+def weights(K: int, F: int, mode: int = AVG_CENTRE_SYMMETRIC) -> np.ndarray:
+    W = np.empty((K // F, K), dtype=np.float64)
+    _check(_load().mwax_oracle_weights(K, F, mode, _dp(W)), "weights")
+    return W
+
+
+def spectra(volt: np.ndarray, N: int, K: int, T: int, dump: int = 0, sel=None) -> np.ndarray:
+    """volt int8 [n][samples][2] -> Y complex128 [K][T][n_sel] (steps 1-3)."""
+    assert volt.dtype == np.int8 and volt.ndim == 3 and volt.shape[2] == 2 and volt.flags.c_contiguous
+    assert volt.shape[1] >= (dump + 1) * T * N
+    s, sp = _sel(sel, volt.shape[0])
+    Y = np.empty((K, T, s.size), dtype=np.complex128)
+    _check(_load().mwax_oracle_spectra(s.size, sp, N, K, T, dump, volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)),
+                                       volt.shape[1], _dp(Y.view(np.float64))), "spectra")
+    return Y
+
+
+def correlate(Y: np.ndarray) -> np.ndarray:
+    """Y complex128 [K][T][n] -> R complex128 [K][n(n+1)/2] (step 4)."""
+    Y = np.ascontiguousarray(Y, dtype=np.complex128)
+    K, T, n = Y.shape
+    R = np.empty((K, n * (n + 1) // 2), dtype=np.complex128)
+    _check(_load().mwax_oracle_correlate(n, K, T, _dp(Y.view(np.float64)), _dp(R.view(np.float64))), "correlate")
+    return R
+
+
+def average(R: np.ndarray, n: int, F: int, mode: int = AVG_CENTRE_SYMMETRIC) -> np.ndarray:
+    """R complex128 [K][B] -> V complex128 [K/F][B] (steps 5-6)."""
+    R = np.ascontiguousarray(R, dtype=np.complex128)
+    K, B = R.shape
+    assert B == n * (n + 1) // 2
+    V = np.empty((K // F, B), dtype=np.complex128)
+    _check(_load().mwax_oracle_average(n, K, F, mode, _dp(R.view(np.float64)), _dp(V.view(np.float64))), "average")
+    return V
+
+
+def fx(volt: np.ndarray, N: int, K: int, T: int, F: int, mode: int = AVG_CENTRE_SYMMETRIC, dump: int = 0,
+       sel=None) -> np.ndarray:
+    """Whole float path, one dump: int8 [n][samples][2] -> V complex128 [K/F][n_sel(n_sel+1)/2]."""
+    assert volt.dtype == np.int8 and volt.ndim == 3 and volt.shape[2] == 2 and volt.flags.c_contiguous
+    assert volt.shape[1] >= (dump + 1) * T * N
+    s, sp = _sel(sel, volt.shape[0])
+    V = np.empty((K // F, s.size * (s.size + 1) // 2), dtype=np.complex128)
+    _check(_load().mwax_oracle_fx(s.size, sp, N, K, T, F, mode, dump,
+                                  volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), volt.shape[1],
+                                  _dp(V.view(np.float64))), "fx")
+    return V
+
+
+def xcorr_i8(z: np.ndarray, sel=None) -> np.ndarray:
+    """z int8 [chan][time][input][2] -> int32 [chan][n_sel(n_sel+1)/2][2], exact."""
+    assert z.dtype == np.int8 and z.ndim == 4 and z.shape[3] == 2 and z.flags.c_contiguous
+    n_chan, n_time, n_inputs, _ = z.shape
+    s, sp = _sel(sel, n_inputs)
+    vis = np.empty((n_chan, s.size * (s.size + 1) // 2, 2), dtype=np.int32)
+    _check(_load().mwax_oracle_xcorr_i8(s.size, sp, n_inputs, n_chan, n_time,
+                                        z.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)),
+                                        vis.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))), "xcorr_i8")
+    return vis
+
+
+def baseline_index(i: int, j: int) -> int:
+    """Packed lower-triangle index of pair (i >= j)."""
+    assert i >= j >= 0
+    return i * (i + 1) // 2 + j

@@ -1,0 +1,344 @@
+"""Pins for the float64 oracle: what the paper and the mathematics fix.
+
+Every check here compares the oracle against something OTHER than itself: a brute-force sum written
+out in numpy, numpy.fft as a library routine on special cases, closed forms, invariants stated in the
+paper, values printed in the paper (tests/golden/), or statistical expectations.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import oracle
+from paper_2303_11557_b200 import synth
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+rng = np.random.default_rng(20231157)
+
+
+def _rand_c(n):
+    return rng.standard_normal(n) + 1j * rng.standard_normal(n)
+
+
+def _brute_dft(x):
+    N = x.size
+    k = np.arange(N)
+    # definition with exact integer phase reduction
+    ph = (np.outer(k, k) % N) / N
+    return (x[None, :] * np.exp(-2j * np.pi * ph)).sum(axis=1)
+
+
+def _volt_from_complex(x):
+    """complex array [n][m] with integer parts -> int8 [n][m][2]"""
+    v = np.empty(x.shape + (2,), dtype=np.int8)
+    v[..., 0] = np.rint(x.real)
+    v[..., 1] = np.rint(x.imag)
+    return v
+
+
+# ------------------------------------------------------------------ P1: DFT routine
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 7, 8, 10, 16, 20, 25, 50, 64, 100, 125, 128, 256, 320, 625, 1000])
+def test_p1_fft_equals_bruteforce(N):
+    x = _rand_c(N)
+    ref = _brute_dft(x)
+    scale = np.abs(ref).max()
+    assert np.abs(oracle.fft(x) - ref).max() <= 1e-10 * scale
+    assert np.abs(oracle.dft_naive(x) - ref).max() <= 1e-10 * scale
+
+
+def test_p1_fft_6400_vs_library_and_sampled_bruteforce():
+    N = 6400
+    x = _rand_c(N)
+    got = oracle.fft(x)
+    lib = np.fft.fft(x)  # library routine, same sign/scale convention (reading Q1)
+    assert np.abs(got - lib).max() <= 1e-10 * np.abs(lib).max()
+    q = np.arange(N)
+    for k in [0, 1, 5, 175, 3199, 3200, 4793, 6399]:
+        bf = (x * np.exp(-2j * np.pi * ((k * q) % N) / N)).sum()
+        assert abs(got[k] - bf) <= 1e-9 * np.abs(lib).max()
+
+
+def test_p1_impulse_and_linearity():
+    N = 100
+    e = np.zeros(N, complex)
+    e[0] = 1
+    assert np.allclose(oracle.fft(e), np.ones(N), atol=1e-13)
+    e[:] = 0
+    e[3] = 1  # shifted impulse -> pure phase ramp exp(-2 pi i 3k/N)
+    assert np.allclose(oracle.fft(e), np.exp(-2j * np.pi * 3 * np.arange(N) / N), atol=1e-12)
+    a, b = _rand_c(N), _rand_c(N)
+    assert np.allclose(oracle.fft(2 * a - 3j * b), 2 * oracle.fft(a) - 3j * oracle.fft(b), atol=1e-10)
+
+
+# ------------------------------------------------------------------ P2: sign + channel map
+@pytest.mark.parametrize("N,K", [(64, 64), (128, 128), (100, 50), (25, 25), (25, 11), (6400, 6400)])
+def test_p2_tone_lands_in_expected_position(N, K):
+    T, A = 2, 20.0
+    q = np.arange(N * T)
+    for k0 in [3, -3, 0]:
+        if abs(k0) > (K - 1) // 2:
+            continue
+        x = A * np.exp(2j * np.pi * ((k0 * q) % N) / N)
+        # exact integer voltages are needed for the int8 interface: use a tone whose samples are integers
+        # only when k0 == 0; otherwise feed the rounded tone and check the dominant position and its phase.
+        Y = oracle.spectra(_volt_from_complex(x[None, :]), N, K, T)
+        p = np.unravel_index(np.abs(Y[:, 0, 0]).argmax(), (K,))[0]
+        assert p == k0 + K // 2  # DC at floor(K/2); +k0 above it; -k0 mirrors below
+        assert abs(Y[p, 0, 0] - A * N) <= 0.02 * A * N  # value A*N up to int8 rounding noise
+    # constant input -> DC position only, exact
+    x = np.full(N * T, 7 + 3j)
+    Y = oracle.spectra(_volt_from_complex(x[None, :]), N, K, T)
+    assert np.allclose(Y[K // 2, :, 0], (7 + 3j) * N, atol=1e-9)
+    Y[K // 2] = 0
+    assert np.abs(Y).max() < 1e-9
+
+
+def test_p2_keep_selects_centre_channels_in_signed_order():
+    N, K, T = 20, 7, 1
+    x = np.rint(10 * _rand_c(N))
+    full = np.fft.fft(x)  # library routine
+    Y = oracle.spectra(_volt_from_complex(x[None, :]), N, K, T)[:, 0, 0]
+    expect = np.array([full[u % N] for u in range(-(K // 2), K - K // 2)])
+    assert np.allclose(Y, expect, atol=1e-10)
+    # even K: the extra channel is on the negative side (reading Q3)
+    K = 8
+    Y = oracle.spectra(_volt_from_complex(x[None, :]), N, K, T)[:, 0, 0]
+    expect = np.array([full[u % N] for u in range(-4, 4)])
+    assert np.allclose(Y, expect, atol=1e-10)
+
+
+# ------------------------------------------------------------------ P3: Parseval
+@pytest.mark.parametrize("N", [64, 128, 50])
+def test_p3_parseval_total_power(N):
+    n, T = 3, 5
+    x = np.rint(16 * (rng.standard_normal((n, N * T)) + 1j * rng.standard_normal((n, N * T))))
+    V = oracle.fx(_volt_from_complex(x), N, N, T, 1)
+    for i in range(n):
+        total = V[:, oracle.baseline_index(i, i)].real.sum()
+        assert abs(total - N * (np.abs(x[i]) ** 2).sum()) <= 1e-9 * total
+
+
+# ------------------------------------------------------------------ P4: correlation structure
+def test_p4_hermitian_autos_and_bruteforce_pairs():
+    n, N, T = 4, 16, 6
+    x = np.rint(16 * (rng.standard_normal((n, N * T)) + 1j * rng.standard_normal((n, N * T))))
+    volt = _volt_from_complex(x)
+    V = oracle.fx(volt, N, N, T, 1)
+    # brute force with numpy.fft (library) + explicit products
+    S = np.fft.fftshift(np.fft.fft(x.reshape(n, T, N), axis=2), axes=2)  # [n][T][p]
+    for i in range(n):
+        for j in range(i + 1):
+            ref = (S[i] * np.conj(S[j])).sum(axis=0)  # over T -> [p]
+            got = V[:, oracle.baseline_index(i, j)]
+            assert np.abs(got - ref).max() <= 1e-9 * np.abs(ref).max()
+    for i in range(n):
+        a = V[:, oracle.baseline_index(i, i)]
+        assert np.all(a.imag == 0.0) and np.all(a.real >= 0.0)
+    # V_ji = conj(V_ij): compute with the input order reversed
+    Vr = oracle.fx(volt, N, N, T, 1, sel=np.arange(n)[::-1])
+    for i in range(n):
+        for j in range(i):
+            # in the reversed selection, input j sits at index n-1-j > n-1-i
+            vji = Vr[:, oracle.baseline_index(n - 1 - j, n - 1 - i)]
+            assert np.allclose(vji, np.conj(V[:, oracle.baseline_index(i, j)]), rtol=1e-12, atol=1e-9)
+
+
+def test_p4_tone_phase_and_amplitude_closure():
+    """§3.1 method: per-input tones of known amplitude/phase -> arg V_ij = phi_i - phi_j and
+    |V_ij| = T N^2 a_i a_j."""
+    n, N, T, k0 = 4, 64, 4, 5
+    amps = np.array([10.0, 20.0, 30.0, 40.0])
+    phis = np.array([0.1, 1.3, -2.0, 2.9])
+    q = np.arange(N * T)
+    x = amps[:, None] * np.exp(1j * (2 * np.pi * ((k0 * q) % N) / N + phis[:, None]))
+    V = oracle.fx(_volt_from_complex(x), N, N, T, 1)
+    p = k0 + N // 2
+    for i in range(n):
+        for j in range(i + 1):
+            v = V[p, oracle.baseline_index(i, j)]
+            assert abs(abs(v) - T * N * N * amps[i] * amps[j]) <= 0.03 * T * N * N * amps[i] * amps[j]
+            d = np.angle(v * np.exp(-1j * (phis[i] - phis[j])))
+            assert abs(d) < 0.03
+
+
+def test_p4_additivity_over_time():
+    n, N, T = 3, 20, 4
+    x = np.rint(16 * (rng.standard_normal((n, N * 2 * T)) + 1j * rng.standard_normal((n, N * 2 * T))))
+    volt = _volt_from_complex(x)
+    whole = oracle.fx(volt, N, N, 2 * T, 1)
+    parts = oracle.fx(volt, N, N, T, 1, dump=0) + oracle.fx(volt, N, N, T, 1, dump=1)
+    assert np.allclose(whole, parts, rtol=1e-12, atol=1e-9)
+
+
+# ------------------------------------------------------------------ P5: common-signal recovery
+def test_p5_common_signal_correlation_coefficient():
+    cfg = synth.CONFIGS["C1"]
+    spec = cfg.spec()
+    spec.tones = []  # exclude tones (an off-bin or strong tone biases r-hat)
+    volt = synth.gauss_voltages(spec)
+    V = oracle.fx(volt, cfg.n_fft, cfg.n_keep, cfg.t_int, 1)
+    n = cfg.n_inputs
+    sigma2 = cfg.sigma ** 2
+    expect = cfg.rho * sigma2 / (sigma2 + 1.0 / 12.0)  # integer rounding adds 1/12 variance per component
+    M = cfg.t_int * cfg.n_keep
+    rs = []
+    for i in range(n):
+        for j in range(i):
+            v = V[:, oracle.baseline_index(i, j)].sum()
+            ai = V[:, oracle.baseline_index(i, i)].real.sum()
+            aj = V[:, oracle.baseline_index(j, j)].real.sum()
+            rs.append(v / np.sqrt(ai * aj))
+    rs = np.array(rs)
+    tol = 5.0 / np.sqrt(M)  # conservative 5 sigma; all baselines share s so they do not average down
+    assert np.all(np.abs(rs.real - expect) < tol)
+    assert np.all(np.abs(rs.imag) < tol)
+    assert abs(rs.real.mean() - expect) < tol
+
+
+# ------------------------------------------------------------------ P6-P8: averaging weights
+def test_weights_golden_K8_F2():
+    tab = np.loadtxt(os.path.join(GOLDEN, "weights_K8_F2.txt"))
+    W = oracle.weights(8, 2)
+    assert np.array_equal(W * 2, tab)  # table is before the division by F
+
+
+@pytest.mark.parametrize("K,F", [(8, 2), (256, 2), (6400, 25), (6400, 50), (6400, 256), (6400, 5), (100, 4), (75, 3)])
+def test_p7_partition_of_unity_and_symmetry(K, F):
+    W = oracle.weights(K, F)
+    C = K // F
+    c0, dc = C // 2, K // 2
+    assert np.allclose(W.sum(axis=1), 1.0)  # rows are means
+    assert np.all(W[:, dc] == 0.0)  # DC column excluded (L290)
+    col = W.sum(axis=0) * F
+    centre_taps = np.nonzero(W[c0])[0]
+    others = np.setdiff1d(np.arange(K), np.concatenate([centre_taps, [dc]]))
+    # "energy at every frequency contributes equally" (L306): total weight 1 outside the re-scaled centre group
+    assert np.allclose(col[others], 1.0)
+    # ends of the centre group are shared with a neighbour at weight 1/2 each side when F is even
+    # mirror symmetry about the centre channel (L296, L302): taps of c0+m mirror those of c0-m about DC
+    for m in range(1, min(c0, C - 1 - c0) + 1):
+        up, dn = W[c0 + m], W[c0 - m]
+        for p in np.nonzero(up)[0]:
+            pm = (2 * dc - p) % K
+            assert dn[pm] == up[p]
+    # tap counts (L298)
+    ntaps = (W[(c0 + 1) % C] != 0).sum() if C > 1 else None
+    if C > 1:
+        assert ntaps == (F if F % 2 else F + 1)
+
+
+def test_p6_boundary_tone_splits_50_50():
+    """An on-bin tone exactly on an output-channel boundary appears at 50 % in each neighbour — 'precisely 3 dB
+    down at the channel boundaries'."""
+    N = K = 400
+    F, T, A = 50, 1, 30.0
+    u = 25 + 50 * 2  # boundary between output channels c0+2 and c0+3
+    q = np.arange(N * T)
+    x = A * np.exp(2j * np.pi * ((u * q) % N) / N)
+    V = oracle.fx(_volt_from_complex(x[None, :]), N, K, T, F)[:, 0].real
+    full = oracle.fx(_volt_from_complex(x[None, :]), N, K, T, 1)[:, 0].real
+    tone_power = full[u + K // 2]
+    c0 = (K // F) // 2
+    lo, hi = V[c0 + 2] * F, V[c0 + 3] * F  # undo the mean
+    assert abs(lo / tone_power - 0.5) < 0.01 and abs(hi / tone_power - 0.5) < 0.01
+    assert abs(10 * np.log10(lo / tone_power) + 3.0103) < 0.1
+
+
+def test_p8_dc_tone_vanishes_and_white_noise_is_flat():
+    N = K = 64
+    F, T = 4, 2000
+    x = np.full(N * 4, 50.0 + 0j)
+    V = oracle.fx(_volt_from_complex(x[None, :]), N, K, 4, F)[:, 0]
+    assert np.abs(V).max() < 1e-6  # a pure DC offset leaves no trace anywhere
+    # white noise: every output channel, including the re-scaled centre one, has the same expected power
+    spec = synth.GaussSpec(1, N * T, N, sigma=16.0, rho=0.0, seed=77)
+    V = oracle.fx(synth.gauss_voltages(spec), N, K, T, F)[:, 0].real
+    expect = T * N * 2 * (16.0 ** 2 + 1 / 12)
+    # relative std of a channel ~ 1/sqrt(T*F) ~ 1.1 % (centre channel: 1/sqrt(T*(F-1)))
+    assert np.all(np.abs(V / expect - 1.0) < 0.06)
+    c0 = (K // F) // 2
+    assert abs(V[c0] / np.delete(V, c0).mean() - 1.0) < 0.05
+
+
+def test_block_mode_weights():
+    W = oracle.weights(12, 3, oracle.AVG_BLOCK)
+    for c in range(4):
+        expect = np.zeros(12)
+        expect[3 * c:3 * c + 3] = 1 / 3
+        assert np.allclose(W[c], expect)
+    assert np.array_equal(oracle.weights(16, 1), np.eye(16))  # F = 1: identity, no DC exclusion (reading Q7)
+
+
+def test_average_equals_weight_table_product():
+    n, K, F = 3, 24, 4
+    B = n * (n + 1) // 2
+    R = _rand_c(K * B).reshape(K, B)
+    V = oracle.average(R, n, F)
+    W = oracle.weights(K, F)
+    ref = W @ R
+    for a in range(n):
+        ref[:, oracle.baseline_index(a, a)] = ref[:, oracle.baseline_index(a, a)].real
+    assert np.allclose(V, ref, rtol=1e-13, atol=1e-13)
+
+
+# ------------------------------------------------------------------ P9: output sizes printed in the paper
+def test_p9_fig14_data_rates():
+    rows = np.loadtxt(os.path.join(GOLDEN, "fig14_rates.txt"))
+    n = 256  # 128 tiles x 2 polarisations
+    for fscrunch, count, tres, rate in rows:
+        assert 6400 // int(fscrunch) == int(count)
+        W = oracle.weights(6400, int(fscrunch)) if fscrunch in (25, 50) else None
+        C = W.shape[0] if W is not None else 6400 // int(fscrunch)
+        nbytes = C * (n * (n + 1) // 2) * 8  # complex fp32 lower triangle incl. autos (Fig 8: "complex single-precision")
+        got = nbytes / tres * 24 / 1e9
+        assert abs(got - rate) <= 0.0051 + 1e-9, (fscrunch, tres, got, rate)
+
+
+def test_fig8_baseline_count():
+    n, rows = np.loadtxt(os.path.join(GOLDEN, "fig8_baseline_rows.txt"), dtype=int)
+    x = np.rint(5 * _rand_c(n * 8)).reshape(n, 8)
+    V = oracle.fx(_volt_from_complex(x), 8, 8, 1, 1)
+    assert V.shape[1] == rows
+    assert oracle.baseline_index(n - 1, n - 1) == rows - 1
+
+
+# ------------------------------------------------------------------ P10: integer path
+def test_p10_int_path_bruteforce_trace_hermitian_and_float_equality():
+    n_chan, n_time, n = 3, 37, 6
+    z = synth.uniform_voltages(n_chan, n_time, n, n_shared=2, seed=5)
+    vis = oracle.xcorr_i8(z)
+    zc = z[..., 0].astype(np.int64) + 1j * z[..., 1].astype(np.int64)  # [c][t][i]
+    for c in range(n_chan):
+        for i in range(n):
+            for j in range(i + 1):
+                ref = (zc[c, :, i] * np.conj(zc[c, :, j])).sum()
+                got = vis[c, oracle.baseline_index(i, j)]
+                assert got[0] == int(ref.real) and got[1] == int(ref.imag)
+        trace = sum(int(vis[c, oracle.baseline_index(i, i), 0]) for i in range(n))
+        assert trace == int((np.abs(zc[c]) ** 2).sum().round())
+        assert all(vis[c, oracle.baseline_index(i, i), 1] == 0 for i in range(n))
+    # equals the float64 step-4 oracle on the same integers, exactly
+    R = oracle.correlate(np.ascontiguousarray(zc.astype(np.complex128)))
+    assert np.array_equal(R.real.astype(np.int64), vis[..., 0]) and np.array_equal(R.imag.astype(np.int64), vis[..., 1])
+    # swapping the two inputs conjugates
+    v01 = oracle.xcorr_i8(z, sel=[0, 1])[:, 1]
+    v10 = oracle.xcorr_i8(z, sel=[1, 0])[:, 1]
+    assert np.array_equal(v01[:, 0], v10[:, 0]) and np.array_equal(v01[:, 1], -v10[:, 1])
+
+
+# ------------------------------------------------------------------ C1 worked expectation
+def test_c1_tone_position_and_phase_gradient():
+    """BASELINE.json configs[0]: tone at bin +5 -> position 37; arg V_jk = 2 pi (j - k)/16."""
+    cfg = synth.CONFIGS["C1"]
+    volt = synth.gauss_voltages(cfg.spec())
+    V = oracle.fx(volt, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg)
+    autos = np.array([V[:, oracle.baseline_index(i, i)].real for i in range(cfg.n_inputs)])
+    assert np.all(autos.argmax(axis=1) == 37)
+    # expected value at the tone position: tone term T N^2 a^2 e^{i dphi} plus the (real) common-signal term
+    T, N, a = cfg.t_int, cfg.n_fft, cfg.tones[0].amp
+    common = cfg.rho * 2 * cfg.sigma ** 2 * N * T
+    for j, k in [(1, 0), (5, 2), (15, 3), (9, 8), (12, 4)]:
+        expect = T * N * N * a * a * np.exp(2j * np.pi * (j - k) / 16) + common
+        got = V[37, oracle.baseline_index(j, k)]
+        assert abs(np.angle(got * np.conj(expect))) < 0.03
+        assert abs(abs(got) / abs(expect) - 1.0) < 0.05
