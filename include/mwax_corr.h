@@ -1,0 +1,132 @@
+/*
+ * mwax_corr.h — C ABI of the B200-native MWAX FX-correlator hot path.
+ *
+ * What the library computes (PAPER.md = Morrison et al., "MWAX: A New Correlator for the Murchison
+ * Widefield Array", arXiv 2303.11557; readings Q1-Q18 are listed in DESIGN.md §3):
+ *
+ *   F stage   PAPER.md §2.5, §2.5.1: every signal path's complex 8-bit voltage stream is cut
+ *             into non-overlapping frames of n_fft samples and each frame is Fourier transformed (forward,
+ *             unnormalised) into n_fft fine channels.  The n_keep channels centred on DC are kept, in
+ *             ascending signed frequency (L290 centre-symmetric; §4.5 L611 discard the rest).
+ *   X stage   §2.1, §2.5.2: for every fine channel, every pair of signal paths (autos
+ *             included) is cross-multiplied, V_ij = sum_t X_i(t) * conj(X_j(t)), and accumulated over the
+ *             integration time (t_int spectra, L280).
+ *   Averaging §2.6: f_avg adjacent fine channels are averaged into one output channel with the
+ *             paper's centre-symmetric grouping (the DC fine channel excluded and its channel re-scaled;
+ *             f_avg+1 taps with half-weighted ends when f_avg is even), or plain adjacent blocks
+ *             (MWAX_AVG_BLOCK, the legacy grouping of Fig. 6a).
+ *
+ * Everything runs in hand-written sm_100a kernels (no cuFFT, no xGPU, no CPU fallback).  All entry points
+ * are plain C: pointers are DEVICE pointers unless the name says `_host`; sizes are in the units stated.
+ * Calls return MWAX_OK (0) or a negative error code; nothing throws, aborts or prints.
+ *
+ * Threading/streams: all device work of a call is enqueued on `stream` (a cudaStream_t passed as void*;
+ * NULL = the legacy default stream) and the call returns after enqueueing.  One call in flight per handle
+ * (the handle owns a workspace); different handles may run on different streams.
+ */
+#ifndef MWAX_CORR_H
+#define MWAX_CORR_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mwax_corr mwax_corr_t;   /* opaque FX plan + workspace */
+typedef struct mwax_xcorr mwax_xcorr_t; /* opaque X-only integer plan */
+
+enum {
+    MWAX_OK = 0,
+    MWAX_ERR_NULL = -1,        /* a required pointer was NULL                                   */
+    MWAX_ERR_INVALID_ARG = -2, /* argument out of range (sizes < 1, misaligned pointer, ...)    */
+    MWAX_ERR_UNSUPPORTED = -3, /* n_fft not 2^a*5^b or > 6400, n_keep > n_fft, f_avg !| n_keep  */
+    MWAX_ERR_NOMEM = -4,       /* host or device allocation failed                              */
+    MWAX_ERR_CUDA = -5,        /* a CUDA runtime/driver call failed; see mwax_corr_last_cuda_error */
+    MWAX_ERR_ARCH = -6         /* no CUDA device, or the current device is not sm_100           */
+};
+
+/* options for mwax_corr_set_option */
+enum { MWAX_OPT_AVG_MODE = 1 };
+enum { MWAX_AVG_CENTRE_SYMMETRIC = 0, MWAX_AVG_BLOCK = 1 };
+
+/* ------------------------------------------------------------------------------------------------------
+ * FX path (BASELINE.json north star).
+ *
+ * mwax_corr_create(n_inputs, n_fft, n_keep, t_int, f_avg)
+ *   n_inputs  number of signal paths n (tiles x 2 polarisations), >= 1
+ *   n_fft     frame / FFT length N; must be 2^a * 5^b, 1 <= N <= 6400 (the paper uses 6400, L264)
+ *   n_keep    K <= N fine channels kept, centred on DC: signed bins u in [-floor(K/2), ceil(K/2)),
+ *             output position p = u + floor(K/2)
+ *   t_int     T >= 1 spectra summed into one integration (seconds never cross the ABI: T = t * 1.28e6 / N)
+ *   f_avg     F >= 1 fine channels per output channel, F | K; C = K/F output channels
+ * Returns a handle owning its tables and an fp16 workspace of mwax_corr_workspace_bytes() on the current
+ * CUDA device, or NULL; the reason is then returned by mwax_corr_last_error() (thread-local).
+ * ---------------------------------------------------------------------------------------------------- */
+mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, int f_avg);
+int mwax_corr_last_error(void);
+
+/* Averaging geometry; call before the first process().  Default MWAX_AVG_CENTRE_SYMMETRIC. */
+int mwax_corr_set_option(mwax_corr_t *h, int key, int value);
+
+/* One integration:
+ *   d_volt  in : int8 [n_inputs][T*N][re,im] — row i is signal path i's contiguous sample stream
+ *                (PAPER.md L260), row pitch exactly T*N samples; two's-complement, -128 accepted.
+ *                Must be 16-byte aligned.  mwax_corr_input_bytes() = n*T*N*2.
+ *   d_vis   out: float [C][n(n+1)/2][re,im], baseline index i*(i+1)/2 + j for i >= j,
+ *                V_ij = sum X_i conj(X_j); autos have Im == 0 exactly; sum (not mean) over time, weighted
+ *                MEAN over the averaged fine channels; DFT unnormalised.  mwax_corr_output_bytes() = C*B*8.
+ * Caller owns both buffers; they must stay valid until the stream has drained.
+ */
+int mwax_corr_process(mwax_corr_t *h, const int8_t *d_volt, float *d_vis, void *stream);
+
+/* Several integrations / coarse channels from one resident buffer, no copies:
+ *   sample (coarse c, input i, time m) is at d_volt + 2*(c*coarse_pitch + i*row_pitch + m) bytes;
+ *   dump d uses samples [d*T*N, (d+1)*T*N) of every row.  Pitches are in complex samples and must keep
+ *   every frame start 16-byte aligned (even pitches when N is a multiple of 8).
+ *   d_vis: float [n_coarse][n_dumps][C][B][2].
+ */
+int mwax_corr_process_batch(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, size_t coarse_pitch,
+                            int n_dumps, int n_coarse, float *d_vis, void *stream);
+
+/* Same as process_batch but with HOST buffers (pinned memory recommended): the call copies the voltages
+ * host->device, runs the path, copies the visibilities device->host, all on `stream`, and synchronises
+ * the stream before returning.  Staging buffers are owned by the handle (allocated on first use). */
+int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitch, size_t coarse_pitch,
+                           int n_dumps, int n_coarse, float *h_vis, void *stream);
+
+/* F stage / X stage on their own (used by the per-stage benchmarks and tests).
+ * f_stage writes the handle's workspace; x_stage consumes it.  Same argument meaning as process(). */
+int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, void *stream);
+int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream);
+
+size_t mwax_corr_input_bytes(const mwax_corr_t *h);
+size_t mwax_corr_output_bytes(const mwax_corr_t *h);
+size_t mwax_corr_workspace_bytes(const mwax_corr_t *h);
+/* number of kernel launches one process() call enqueues */
+int mwax_corr_launches_per_process(const mwax_corr_t *h);
+int mwax_corr_last_cuda_error(const mwax_corr_t *h);
+int mwax_corr_destroy(mwax_corr_t *h); /* NULL is a no-op returning MWAX_OK */
+
+/* ------------------------------------------------------------------------------------------------------
+ * X-only integer path (BASELINE.json configs[1]): the X-stage contraction on pre-channelised int8
+ * samples, exact int32 accumulation, no FFT, no averaging.
+ *   d_z   in : int8 [n_chan][n_time][n_inputs][re,im]; n_inputs must be a multiple of 8 (TMA needs a
+ *              16-byte row pitch) and d_z 16-byte aligned
+ *   d_vis out: int32 [n_chan][n(n+1)/2][re,im],  Re = sum(a_i a_j + b_i b_j), Im = sum(b_i a_j - a_i b_j)
+ * The caller guarantees 2*128*128*n_time < 2^31 (n_time <= 65535) so int32 cannot overflow.
+ * ---------------------------------------------------------------------------------------------------- */
+mwax_xcorr_t *mwax_xcorr_i8_create(int n_inputs, int n_chan, int n_time);
+int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, void *stream);
+int mwax_xcorr_i8_process_host(mwax_xcorr_t *h, const int8_t *h_z, int32_t *h_vis, void *stream);
+int mwax_xcorr_i8_destroy(mwax_xcorr_t *h);
+
+const char *mwax_corr_strerror(int code);
+/* "sm_100a tcgen05/TMA; built <date>" — identifies the native library in logs */
+const char *mwax_corr_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MWAX_CORR_H */

@@ -1,0 +1,171 @@
+// f_stage.cuh — F stage: int8 complex voltages -> FFT -> keep/centre-order -> scale -> fp16, written already
+// corner-turned into the X stage's operand layout Y[p][t][input][re,im] (no separate transpose pass).
+//
+// PAPER.md §2.5, §2.5.1 L264 (promote 8-bit to float, FFT), L274 (transpose), L290/L611 (centre order,
+// keep); DESIGN.md §5.1.
+//
+// Generic kernel (any N = 2^a 5^b): one CTA transforms one frame of G adjacent inputs with a Stockham autosort
+// FFT in shared memory, radix 4/2/5 passes, fp32.  The G transforms are interleaved in shared memory
+// ([index][g], g fastest) so that a warp's accesses are conflict free and the final store writes G*4
+// contiguous bytes per (channel, time) row.
+#pragma once
+#include <cuda_fp16.h>
+#include <cstdint>
+
+namespace mwax {
+
+struct FParams {
+    const int8_t *volt;      // [input][row_pitch samples][re,im]
+    long long row_pitch;     // samples
+    long long sample0;       // first sample of this dump in every row
+    int n_inputs, N, K, T;
+    int G;                   // inputs per CTA
+    int n_pass;
+    int radix[16];
+    int vec_ok;              // 16-byte loads allowed
+    const float2 *tw;        // [N] exp(-2 pi i m / N)
+    const float *sw;         // [K] per-position factor: s * sqrt(w_p)
+    __half2 *Y;              // [K][T][pitch2]
+    int pitch2;              // half2 (complex) elements per Y row
+};
+
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+
+// y_k = sum_j x_j w_R^{jk}, forward (w_R = exp(-2 pi i / R))
+template <int R>
+__device__ __forceinline__ void butterfly(float2 (&x)[R]);
+
+template <>
+__device__ __forceinline__ void butterfly<2>(float2 (&x)[2])
+{
+    const float2 a = x[0], b = x[1];
+    x[0] = make_float2(a.x + b.x, a.y + b.y);
+    x[1] = make_float2(a.x - b.x, a.y - b.y);
+}
+template <>
+__device__ __forceinline__ void butterfly<4>(float2 (&x)[4])
+{
+    const float2 a = make_float2(x[0].x + x[2].x, x[0].y + x[2].y);
+    const float2 b = make_float2(x[0].x - x[2].x, x[0].y - x[2].y);
+    const float2 c = make_float2(x[1].x + x[3].x, x[1].y + x[3].y);
+    const float2 d = make_float2(x[1].x - x[3].x, x[1].y - x[3].y);
+    x[0] = make_float2(a.x + c.x, a.y + c.y);
+    x[2] = make_float2(a.x - c.x, a.y - c.y);
+    x[1] = make_float2(b.x + d.y, b.y - d.x);   // b - i d
+    x[3] = make_float2(b.x - d.y, b.y + d.x);   // b + i d
+}
+template <>
+__device__ __forceinline__ void butterfly<5>(float2 (&x)[5])
+{
+    const float c1 = 0.30901699437494742f, c2 = -0.80901699437494742f;   // cos(2pi/5), cos(4pi/5)
+    const float s1 = 0.95105651629515357f, s2 = 0.58778525229247313f;    // sin(2pi/5), sin(4pi/5)
+    const float2 t1 = make_float2(x[1].x + x[4].x, x[1].y + x[4].y);
+    const float2 t2 = make_float2(x[2].x + x[3].x, x[2].y + x[3].y);
+    const float2 t3 = make_float2(x[1].x - x[4].x, x[1].y - x[4].y);
+    const float2 t4 = make_float2(x[2].x - x[3].x, x[2].y - x[3].y);
+    const float2 m1 = make_float2(x[0].x + c1 * t1.x + c2 * t2.x, x[0].y + c1 * t1.y + c2 * t2.y);
+    const float2 m2 = make_float2(x[0].x + c2 * t1.x + c1 * t2.x, x[0].y + c2 * t1.y + c1 * t2.y);
+    const float2 n1 = make_float2(s1 * t3.x + s2 * t4.x, s1 * t3.y + s2 * t4.y);
+    const float2 n2 = make_float2(s2 * t3.x - s1 * t4.x, s2 * t3.y - s1 * t4.y);
+    x[0] = make_float2(x[0].x + t1.x + t2.x, x[0].y + t1.y + t2.y);
+    x[1] = make_float2(m1.x + n1.y, m1.y - n1.x);   // m1 - i n1
+    x[4] = make_float2(m1.x - n1.y, m1.y + n1.x);   // m1 + i n1
+    x[2] = make_float2(m2.x + n2.y, m2.y - n2.x);
+    x[3] = make_float2(m2.x - n2.y, m2.y + n2.x);
+}
+
+// One Stockham pass over G interleaved transforms:
+//   y[q + s(R p + k)] = w_n^{p k} * sum_j x[q + s(p + m j)] w_R^{j k},  n = current sub-length, m = n/R, b = q + s p
+template <int R>
+__device__ __forceinline__ void stockham_pass(const float2 *__restrict__ src, float2 *__restrict__ dst, int N, int G,
+                                              int n_cur, int s, const float2 *__restrict__ tw)
+{
+    const int nb = N / R;
+    const int tw_step = N / n_cur;
+    for (int w = threadIdx.x; w < nb * G; w += blockDim.x) {
+        const int g = w % G, b = w / G;
+        const int p = b / s, q = b - p * s;
+        float2 x[R];
+#pragma unroll
+        for (int j = 0; j < R; ++j) x[j] = src[(b + j * nb) * G + g];
+        butterfly<R>(x);
+        const int o = q + s * R * p;
+        dst[o * G + g] = x[0];
+#pragma unroll
+        for (int k = 1; k < R; ++k) dst[(o + s * k) * G + g] = cmul(x[k], __ldg(&tw[p * k * tw_step]));
+    }
+}
+
+__global__ void __launch_bounds__(256) f_stage_generic_kernel(const FParams P)
+{
+    extern __shared__ float2 fbuf[];
+    const int G = P.G, N = P.N;
+    float2 *buf0 = fbuf, *buf1 = fbuf + (size_t)G * N;
+    const int i0 = blockIdx.x * G;
+    const int t = blockIdx.y;
+    const long long s_off = P.sample0 + (long long)t * N;
+
+    // ---- load + promote int8 -> fp32, transposing into [q][g]
+    if (P.vec_ok) {
+        const int nv = N / 8;
+        for (int w = threadIdx.x; w < nv * G; w += blockDim.x) {
+            const int g = w % G, v = w / G;
+            const int i = i0 + g;
+            int4 raw = make_int4(0, 0, 0, 0);
+            if (i < P.n_inputs)
+                raw = __ldg(reinterpret_cast<const int4 *>(P.volt + 2 * ((long long)i * P.row_pitch + s_off + 8 * v)));
+            const int wd[4] = {raw.x, raw.y, raw.z, raw.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const int x = wd[e];
+                buf0[(8 * v + 2 * e) * G + g] = make_float2((float)(int8_t)(x & 0xff), (float)(int8_t)((x >> 8) & 0xff));
+                buf0[(8 * v + 2 * e + 1) * G + g] =
+                    make_float2((float)(int8_t)((x >> 16) & 0xff), (float)(int8_t)((x >> 24) & 0xff));
+            }
+        }
+    } else {
+        for (int w = threadIdx.x; w < N * G; w += blockDim.x) {
+            const int g = w % G, qq = w / G;
+            const int i = i0 + g;
+            float2 v = make_float2(0.f, 0.f);
+            if (i < P.n_inputs) {
+                const int8_t *s = P.volt + 2 * ((long long)i * P.row_pitch + s_off + qq);
+                v = make_float2((float)s[0], (float)s[1]);
+            }
+            buf0[qq * G + g] = v;
+        }
+    }
+    __syncthreads();
+
+    // ---- FFT passes
+    float2 *src = buf0, *dst = buf1;
+    int n_cur = N, s = 1;
+    for (int ps = 0; ps < P.n_pass; ++ps) {
+        const int R = P.radix[ps];
+        if (R == 4) stockham_pass<4>(src, dst, N, G, n_cur, s, P.tw);
+        else if (R == 2) stockham_pass<2>(src, dst, N, G, n_cur, s, P.tw);
+        else stockham_pass<5>(src, dst, N, G, n_cur, s, P.tw);
+        n_cur /= R;
+        s *= R;
+        float2 *tmp = src; src = dst; dst = tmp;
+        __syncthreads();
+    }
+
+    // ---- keep the central K channels in signed order, scale, fp16 (round to nearest even), corner-turned store
+    const int half = P.K / 2;
+    for (int w = threadIdx.x; w < P.K * G; w += blockDim.x) {
+        const int g = w % G, p = w / G;
+        const int i = i0 + g;
+        if (i >= P.n_inputs) continue;
+        int k = p - half;
+        if (k < 0) k += N;
+        const float f = __ldg(&P.sw[p]);
+        const float2 v = src[k * G + g];
+        P.Y[((long long)p * P.T + t) * P.pitch2 + i] = __floats2half2_rn(v.x * f, v.y * f);
+    }
+}
+
+}  // namespace mwax

@@ -1,0 +1,482 @@
+// mwax_api.cu — the C ABI (include/mwax_corr.h): plan construction (tables, workspace, TMA tensor maps,
+// triangle tile schedule) and kernel launches.  No CPU fallback: without an sm_100 device create() fails with
+// MWAX_ERR_ARCH.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/mwax_corr.h"
+#include "f_stage.cuh"
+#include "x_stage.cuh"
+
+namespace {
+
+thread_local int g_last_error = MWAX_OK;
+
+typedef CUresult (*PFN_encodeTiled)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+PFN_encodeTiled get_encode_fn()
+{
+    static PFN_encodeTiled fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<PFN_encodeTiled>(p);
+    }
+    return fn;
+}
+
+// 3-D map over rows of `row_bytes` bytes: dims (inner elements, rows per channel, channels); box = 128 bytes x
+// box_rows x 1, SWIZZLE_128B, out-of-bounds elements read as zero (that is what pads partial tiles and the
+// last contraction block of a channel).
+int encode_z_map(CUtensorMap *m, bool int8, const void *base, uint64_t inner_elems, uint64_t row_bytes, uint64_t rows,
+                 uint64_t chans, uint32_t box_rows)
+{
+    PFN_encodeTiled fn = get_encode_fn();
+    if (!fn) return MWAX_ERR_CUDA;
+    cuuint64_t dims[3] = {inner_elems, rows, chans};
+    cuuint64_t strides[2] = {row_bytes, row_bytes * rows};
+    cuuint32_t box[3] = {int8 ? 128u : 64u, box_rows, 1u};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(m, int8 ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 3,
+                    const_cast<void *>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                    CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? MWAX_OK : MWAX_ERR_CUDA;
+}
+
+bool factor_2_5(int N, std::vector<int> &radix)
+{
+    radix.clear();
+    while (N % 4 == 0) { radix.push_back(4); N /= 4; }
+    while (N % 2 == 0) { radix.push_back(2); N /= 2; }
+    while (N % 5 == 0) { radix.push_back(5); N /= 5; }
+    return N == 1;
+}
+
+int check_device(int *sm_count)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return MWAX_ERR_ARCH;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return MWAX_ERR_ARCH;
+    if (prop.major != 10) return MWAX_ERR_ARCH;
+    *sm_count = prop.multiProcessorCount;
+    return MWAX_OK;
+}
+
+// lower-triangle tile list: G-tile (mi, nj) covers inputs i in [64 mi, 64 mi + 64), j in [bn/2 nj, bn/2 (nj+1))
+void build_tiles(int n, int bn, std::vector<uint8_t> &tiles)
+{
+    tiles.clear();
+    const int im = 64, jn = bn / 2;
+    for (int mi = 0; mi * im < n; ++mi)
+        for (int nj = 0; nj * jn < n; ++nj)
+            if (mi * im + im - 1 >= nj * jn) {
+                tiles.push_back((uint8_t)mi);
+                tiles.push_back((uint8_t)nj);
+            }
+}
+
+template <typename T>
+int upload(T **dptr, const std::vector<T> &h)
+{
+    if (*dptr) { cudaFree(*dptr); *dptr = nullptr; }
+    if (cudaMalloc(reinterpret_cast<void **>(dptr), h.size() * sizeof(T)) != cudaSuccess) return MWAX_ERR_NOMEM;
+    if (cudaMemcpy(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice) != cudaSuccess) return MWAX_ERR_CUDA;
+    return MWAX_OK;
+}
+
+template <bool kInt8, int BN>
+int launch_x(const CUtensorMap &tmap, const mwax::XParams &xp, int sm_count, cudaStream_t st)
+{
+    using C = mwax::XConfig<kInt8, BN>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(mwax::x_stage_kernel<kInt8, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 C::SMEM_BYTES) != cudaSuccess)
+            return MWAX_ERR_CUDA;
+        attr_set = true;
+    }
+    const int n_items = xp.n_out * xp.n_tiles;
+    if (n_items <= 0) return MWAX_OK;
+    const int grid = n_items < sm_count ? n_items : sm_count;
+    mwax::x_stage_kernel<kInt8, BN><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(tmap, xp);
+    return cudaGetLastError() == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------ handles
+struct mwax_corr {
+    int n, N, K, T, F, C;
+    int avg_mode;
+    int x_bn;          // X tile width in G columns (128 or 256)
+    int pitch;         // fp16 elements per Y row (2n rounded up to 64)
+    int sm_count;
+    int last_cuda;
+    bool tables_ready;
+    // F plan
+    int G;
+    size_t f_smem;
+    std::vector<int> radix;
+    // device tables
+    float2 *d_tw;
+    float *d_sw;
+    int *d_tap_start;
+    float *d_scale;
+    uint8_t *d_tiles;
+    int n_tiles, n_taps;
+    __half *d_Y;
+    size_t y_bytes;
+    CUtensorMap tmap;
+    // staging for process_host
+    int8_t *d_in;
+    size_t in_bytes;
+    float *d_out;
+    size_t out_bytes;
+};
+
+struct mwax_xcorr {
+    int n, n_chan, n_time;
+    int x_bn;
+    int sm_count;
+    int last_cuda;
+    int *d_tap_start;
+    uint8_t *d_tiles;
+    int n_tiles;
+    int8_t *d_in;
+    int32_t *d_out;
+};
+
+static int note_cuda(int *slot)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) { *slot = (int)e; return MWAX_ERR_CUDA; }
+    return MWAX_OK;
+}
+
+static void free_tables(mwax_corr *h)
+{
+    cudaFree(h->d_sw); h->d_sw = nullptr;
+    cudaFree(h->d_tap_start); h->d_tap_start = nullptr;
+    cudaFree(h->d_scale); h->d_scale = nullptr;
+    cudaFree(h->d_tiles); h->d_tiles = nullptr;
+    h->tables_ready = false;
+}
+
+// Averaging geometry -> per-position factor sw[p], per-channel first tap and epilogue scale.
+// The weights of PAPER.md L290-298 are folded as  W[c][p] = scale_c * s^2-normalised sw[p]^2 :
+//   sw[p]   = s * sqrt(w_p), w_p = 1 inside a group, 1/2 on a shared edge (even F), 0 for the DC fine channel (F > 1)
+//   scale_c = 1/(s^2 F), times F/(F-1) for the centre channel when F > 1.
+static int build_tables(mwax_corr *h)
+{
+    free_tables(h);
+    const int K = h->K, F = h->F, C = h->C;
+    const int lg = (int)std::ceil(std::log2((double)h->N) / 2.0);
+    const double s = std::ldexp(1.0, -lg);   // power of two near 1/sqrt(N): keeps fp16 in range, epilogue exact
+    std::vector<float> sw(K, (float)s), scale(C, (float)(1.0 / (s * s * F)));
+    std::vector<int> tap(C);
+    if (h->avg_mode == MWAX_AVG_BLOCK || F == 1) {
+        h->n_taps = F;
+        for (int c = 0; c < C; ++c) tap[c] = c * F;
+    } else {
+        const int c0 = C / 2, half = K / 2;
+        const int dmax = (F % 2) ? (F - 1) / 2 : F / 2;
+        h->n_taps = 2 * dmax + 1;
+        for (int c = 0; c < C; ++c) {
+            const int u0 = (c - c0) * F - dmax;
+            tap[c] = ((u0 + half) % K + K) % K;
+        }
+        if (F % 2 == 0)
+            for (int p = 0; p < K; ++p) {
+                const int u = p - half;
+                if ((((u - F / 2) % F) + F) % F == 0) sw[p] = (float)(s * std::sqrt(0.5));
+            }
+        sw[half] = 0.0f;                                            // DC excluded (L290-294)
+        scale[c0] = (float)((1.0 / (s * s * F)) * (double)F / (double)(F - 1));
+    }
+    std::vector<uint8_t> tiles;
+    build_tiles(h->n, h->x_bn, tiles);
+    h->n_tiles = (int)tiles.size() / 2;
+    int rc;
+    if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
+    if ((rc = upload(&h->d_tap_start, tap)) != MWAX_OK) return rc;
+    if ((rc = upload(&h->d_scale, scale)) != MWAX_OK) return rc;
+    if ((rc = upload(&h->d_tiles, tiles)) != MWAX_OK) return rc;
+    h->tables_ready = true;
+    return MWAX_OK;
+}
+
+extern "C" {
+
+int mwax_corr_last_error(void) { return g_last_error; }
+
+const char *mwax_corr_strerror(int code)
+{
+    switch (code) {
+        case MWAX_OK: return "ok";
+        case MWAX_ERR_NULL: return "null pointer";
+        case MWAX_ERR_INVALID_ARG: return "invalid argument";
+        case MWAX_ERR_UNSUPPORTED: return "unsupported configuration";
+        case MWAX_ERR_NOMEM: return "out of memory";
+        case MWAX_ERR_CUDA: return "CUDA error";
+        case MWAX_ERR_ARCH: return "no sm_100 CUDA device";
+        default: return "unknown error";
+    }
+}
+
+const char *mwax_corr_version(void) { return "mwax_corr sm_100a tcgen05/TMA; built " __DATE__ " " __TIME__; }
+
+mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, int f_avg)
+{
+    g_last_error = MWAX_OK;
+    if (n_inputs < 1 || n_fft < 1 || n_keep < 1 || t_int < 1 || f_avg < 1) { g_last_error = MWAX_ERR_INVALID_ARG; return nullptr; }
+    std::vector<int> radix;
+    if (n_fft > 6400 || !factor_2_5(n_fft, radix) || n_keep > n_fft || n_keep % f_avg != 0 || n_inputs > 8128) {
+        g_last_error = MWAX_ERR_UNSUPPORTED;
+        return nullptr;
+    }
+    int sm = 0;
+    if ((g_last_error = check_device(&sm)) != MWAX_OK) return nullptr;
+    mwax_corr *h = new (std::nothrow) mwax_corr();
+    if (!h) { g_last_error = MWAX_ERR_NOMEM; return nullptr; }
+    h->n = n_inputs; h->N = n_fft; h->K = n_keep; h->T = t_int; h->F = f_avg; h->C = n_keep / f_avg;
+    h->avg_mode = MWAX_AVG_CENTRE_SYMMETRIC;
+    h->x_bn = 256;
+    if (const char *e = getenv("MWAX_X_TILE_N")) { if (atoi(e) == 128) h->x_bn = 128; }
+    h->pitch = ((2 * n_inputs + 63) / 64) * 64;
+    h->sm_count = sm;
+    h->last_cuda = 0;
+    h->radix = radix;
+    // F plan: as many adjacent inputs per CTA as fit (two fp32 ping-pong buffers), up to 32 (128-byte segments)
+    int G = 32;
+    while (G > 1 && (size_t)2 * G * n_fft * sizeof(float2) > 200 * 1024) G >>= 1;
+    h->G = G;
+    h->f_smem = (size_t)2 * G * n_fft * sizeof(float2);
+    if (cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)h->f_smem) != cudaSuccess) {
+        g_last_error = MWAX_ERR_CUDA; delete h; return nullptr;
+    }
+    // twiddles exp(-2 pi i m / N), computed in double
+    std::vector<float2> tw(n_fft);
+    for (int m = 0; m < n_fft; ++m) {
+        const double a = 2.0 * M_PI * (double)m / (double)n_fft;
+        tw[m] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
+    }
+    if ((g_last_error = upload(&h->d_tw, tw)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
+    // workspace Y[K][T][pitch] fp16, zeroed once (pad columns stay zero)
+    h->y_bytes = (size_t)n_keep * t_int * h->pitch * sizeof(__half);
+    if (cudaMalloc(reinterpret_cast<void **>(&h->d_Y), h->y_bytes) != cudaSuccess) {
+        g_last_error = MWAX_ERR_NOMEM; mwax_corr_destroy(h); return nullptr;
+    }
+    cudaMemset(h->d_Y, 0, h->y_bytes);
+    if ((g_last_error = encode_z_map(&h->tmap, false, h->d_Y, (uint64_t)h->pitch, (uint64_t)h->pitch * 2,
+                                     (uint64_t)t_int, (uint64_t)n_keep, 64)) != MWAX_OK) {
+        mwax_corr_destroy(h); return nullptr;
+    }
+    if ((g_last_error = build_tables(h)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
+    if (cudaDeviceSynchronize() != cudaSuccess) { g_last_error = MWAX_ERR_CUDA; mwax_corr_destroy(h); return nullptr; }
+    return h;
+}
+
+int mwax_corr_set_option(mwax_corr_t *h, int key, int value)
+{
+    if (!h) return MWAX_ERR_NULL;
+    if (key == MWAX_OPT_AVG_MODE) {
+        if (value != MWAX_AVG_CENTRE_SYMMETRIC && value != MWAX_AVG_BLOCK) return MWAX_ERR_INVALID_ARG;
+        h->avg_mode = value;
+        return build_tables(h);
+    }
+    return MWAX_ERR_INVALID_ARG;
+}
+
+int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, void *stream)
+{
+    if (!h || !d_volt) return MWAX_ERR_NULL;
+    if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
+    mwax::FParams fp;
+    fp.volt = d_volt; fp.row_pitch = (long long)row_pitch; fp.sample0 = 0;
+    fp.n_inputs = h->n; fp.N = h->N; fp.K = h->K; fp.T = h->T; fp.G = h->G;
+    fp.n_pass = (int)h->radix.size();
+    for (int i = 0; i < fp.n_pass; ++i) fp.radix[i] = h->radix[i];
+    fp.vec_ok = (h->N % 8 == 0) && (row_pitch % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_volt) & 15u) == 0);
+    fp.tw = h->d_tw; fp.sw = h->d_sw;
+    fp.Y = reinterpret_cast<__half2 *>(h->d_Y); fp.pitch2 = h->pitch / 2;
+    dim3 grid((h->n + h->G - 1) / h->G, h->T);
+    mwax::f_stage_generic_kernel<<<grid, 256, h->f_smem, (cudaStream_t)stream>>>(fp);
+    return note_cuda(&h->last_cuda);
+}
+
+int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
+{
+    if (!h || !d_vis) return MWAX_ERR_NULL;
+    if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
+    mwax::XParams xp;
+    xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = h->C; xp.n_tiles = h->n_tiles;
+    xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = h->n_taps; xp.scale = h->d_scale;
+    xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    int rc = (h->x_bn == 128) ? launch_x<false, 128>(h->tmap, xp, h->sm_count, (cudaStream_t)stream)
+                              : launch_x<false, 256>(h->tmap, xp, h->sm_count, (cudaStream_t)stream);
+    if (rc != MWAX_OK) note_cuda(&h->last_cuda);
+    return rc;
+}
+
+int mwax_corr_process_batch(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, size_t coarse_pitch, int n_dumps,
+                            int n_coarse, float *d_vis, void *stream)
+{
+    if (!h || !d_volt || !d_vis) return MWAX_ERR_NULL;
+    if (n_dumps < 1 || n_coarse < 1 || row_pitch < (size_t)n_dumps * h->T * h->N) return MWAX_ERR_INVALID_ARG;
+    const size_t dump_samples = (size_t)h->T * h->N;
+    const size_t vis_floats = (size_t)h->C * ((size_t)h->n * (h->n + 1) / 2) * 2;
+    for (int c = 0; c < n_coarse; ++c)
+        for (int d = 0; d < n_dumps; ++d) {
+            int rc = mwax_corr_f_stage(h, d_volt + 2 * (c * coarse_pitch + d * dump_samples), row_pitch, stream);
+            if (rc != MWAX_OK) return rc;
+            rc = mwax_corr_x_stage(h, d_vis + ((size_t)c * n_dumps + d) * vis_floats, stream);
+            if (rc != MWAX_OK) return rc;
+        }
+    return MWAX_OK;
+}
+
+int mwax_corr_process(mwax_corr_t *h, const int8_t *d_volt, float *d_vis, void *stream)
+{
+    if (!h) return MWAX_ERR_NULL;
+    return mwax_corr_process_batch(h, d_volt, (size_t)h->T * h->N, 0, 1, 1, d_vis, stream);
+}
+
+int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitch, size_t coarse_pitch, int n_dumps,
+                           int n_coarse, float *h_vis, void *stream)
+{
+    if (!h || !h_volt || !h_vis) return MWAX_ERR_NULL;
+    if (n_dumps < 1 || n_coarse < 1 || row_pitch < (size_t)n_dumps * h->T * h->N) return MWAX_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t row_samples = (size_t)n_dumps * h->T * h->N;
+    const size_t in_bytes = (size_t)h->n * row_samples * 2;
+    const size_t out_bytes = (size_t)n_dumps * mwax_corr_output_bytes(h);
+    if (h->in_bytes < in_bytes) {
+        cudaFree(h->d_in); h->d_in = nullptr; h->in_bytes = 0;
+        if (cudaMalloc(reinterpret_cast<void **>(&h->d_in), in_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
+        h->in_bytes = in_bytes;
+    }
+    if (h->out_bytes < out_bytes) {
+        cudaFree(h->d_out); h->d_out = nullptr; h->out_bytes = 0;
+        if (cudaMalloc(reinterpret_cast<void **>(&h->d_out), out_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
+        h->out_bytes = out_bytes;
+    }
+    for (int c = 0; c < n_coarse; ++c) {
+        if (cudaMemcpy2DAsync(h->d_in, row_samples * 2, h_volt + 2 * c * coarse_pitch, row_pitch * 2, row_samples * 2,
+                              h->n, cudaMemcpyHostToDevice, st) != cudaSuccess)
+            return note_cuda(&h->last_cuda);
+        int rc = mwax_corr_process_batch(h, h->d_in, row_samples, 0, n_dumps, 1, h->d_out, st);
+        if (rc != MWAX_OK) return rc;
+        if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c * out_bytes, h->d_out, out_bytes,
+                            cudaMemcpyDeviceToHost, st) != cudaSuccess)
+            return note_cuda(&h->last_cuda);
+    }
+    if (cudaStreamSynchronize(st) != cudaSuccess) return note_cuda(&h->last_cuda);
+    return MWAX_OK;
+}
+
+size_t mwax_corr_input_bytes(const mwax_corr_t *h) { return h ? (size_t)h->n * h->T * h->N * 2 : 0; }
+size_t mwax_corr_output_bytes(const mwax_corr_t *h)
+{
+    return h ? (size_t)h->C * ((size_t)h->n * (h->n + 1) / 2) * 8 : 0;
+}
+size_t mwax_corr_workspace_bytes(const mwax_corr_t *h) { return h ? h->y_bytes : 0; }
+int mwax_corr_launches_per_process(const mwax_corr_t *h) { return h ? 2 : 0; }
+int mwax_corr_last_cuda_error(const mwax_corr_t *h) { return h ? h->last_cuda : 0; }
+
+int mwax_corr_destroy(mwax_corr_t *h)
+{
+    if (!h) return MWAX_OK;
+    free_tables(h);
+    cudaFree(h->d_tw);
+    cudaFree(h->d_Y);
+    cudaFree(h->d_in);
+    cudaFree(h->d_out);
+    delete h;
+    return MWAX_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ int8 X-only
+mwax_xcorr_t *mwax_xcorr_i8_create(int n_inputs, int n_chan, int n_time)
+{
+    g_last_error = MWAX_OK;
+    if (n_inputs < 1 || n_chan < 1 || n_time < 1) { g_last_error = MWAX_ERR_INVALID_ARG; return nullptr; }
+    if (n_inputs % 8 != 0 || n_inputs > 8128 || n_time > 65535) { g_last_error = MWAX_ERR_UNSUPPORTED; return nullptr; }
+    int sm = 0;
+    if ((g_last_error = check_device(&sm)) != MWAX_OK) return nullptr;
+    mwax_xcorr *h = new (std::nothrow) mwax_xcorr();
+    if (!h) { g_last_error = MWAX_ERR_NOMEM; return nullptr; }
+    h->n = n_inputs; h->n_chan = n_chan; h->n_time = n_time; h->sm_count = sm; h->last_cuda = 0;
+    h->x_bn = 256;
+    if (const char *e = getenv("MWAX_X_TILE_N")) { if (atoi(e) == 128) h->x_bn = 128; }
+    std::vector<int> tap(n_chan);
+    for (int c = 0; c < n_chan; ++c) tap[c] = c;
+    std::vector<uint8_t> tiles;
+    build_tiles(n_inputs, h->x_bn, tiles);
+    h->n_tiles = (int)tiles.size() / 2;
+    if ((g_last_error = upload(&h->d_tap_start, tap)) != MWAX_OK ||
+        (g_last_error = upload(&h->d_tiles, tiles)) != MWAX_OK) {
+        mwax_xcorr_i8_destroy(h); return nullptr;
+    }
+    return h;
+}
+
+int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, void *stream)
+{
+    if (!h || !d_z || !d_vis) return MWAX_ERR_NULL;
+    if (reinterpret_cast<uintptr_t>(d_z) & 15u) return MWAX_ERR_INVALID_ARG;
+    CUtensorMap tmap;
+    int rc = encode_z_map(&tmap, true, d_z, (uint64_t)2 * h->n, (uint64_t)2 * h->n, (uint64_t)h->n_time,
+                          (uint64_t)h->n_chan, 128);
+    if (rc != MWAX_OK) return rc;
+    mwax::XParams xp;
+    xp.n_inputs = h->n; xp.T = h->n_time; xp.K = h->n_chan; xp.n_out = h->n_chan; xp.n_tiles = h->n_tiles;
+    xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = 1; xp.scale = nullptr;
+    xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    rc = (h->x_bn == 128) ? launch_x<true, 128>(tmap, xp, h->sm_count, (cudaStream_t)stream)
+                          : launch_x<true, 256>(tmap, xp, h->sm_count, (cudaStream_t)stream);
+    if (rc != MWAX_OK) note_cuda(&h->last_cuda);
+    return rc;
+}
+
+int mwax_xcorr_i8_process_host(mwax_xcorr_t *h, const int8_t *h_z, int32_t *h_vis, void *stream)
+{
+    if (!h || !h_z || !h_vis) return MWAX_ERR_NULL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t in_bytes = (size_t)h->n_chan * h->n_time * h->n * 2;
+    const size_t out_bytes = (size_t)h->n_chan * ((size_t)h->n * (h->n + 1) / 2) * 8;
+    if (!h->d_in && cudaMalloc(reinterpret_cast<void **>(&h->d_in), in_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
+    if (!h->d_out && cudaMalloc(reinterpret_cast<void **>(&h->d_out), out_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
+    if (cudaMemcpyAsync(h->d_in, h_z, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return note_cuda(&h->last_cuda);
+    int rc = mwax_xcorr_i8_process(h, h->d_in, h->d_out, st);
+    if (rc != MWAX_OK) return rc;
+    if (cudaMemcpyAsync(h_vis, h->d_out, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return note_cuda(&h->last_cuda);
+    if (cudaStreamSynchronize(st) != cudaSuccess) return note_cuda(&h->last_cuda);
+    return MWAX_OK;
+}
+
+int mwax_xcorr_i8_destroy(mwax_xcorr_t *h)
+{
+    if (!h) return MWAX_OK;
+    cudaFree(h->d_tap_start);
+    cudaFree(h->d_tiles);
+    cudaFree(h->d_in);
+    cudaFree(h->d_out);
+    delete h;
+    return MWAX_OK;
+}
+
+}  // extern "C"
