@@ -1,0 +1,315 @@
+#!/usr/bin/env python
+"""bench.py — MWAX FX hot path on B200: real-time 1.28 MHz coarse channels per GPU at 512 inputs.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C3|C4] [--impl ours|reference]
+
+A step = one pass of the whole hot path (F stage -> X stage with fused integration/averaging/triangle store)
+over one batch: `seconds_of_data` of one 512-input coarse channel (BASELINE.json configs[2] "C3" = 10 kHz mode,
+configs[3] "C4" = the paper's 200 Hz x fscrunch 50 mode), all dumps of the batch.  Inputs are seeded synthetic
+voltages (paper_2303_11557_b200.synth) resident in HBM before the timed region; the e2e leg
+repeats the measurement through mwax_corr_process_host with pinned HOST buffers (H2D + D2H inside the timed
+region).  N > 1: one process per GPU (torchrun), every rank correlates its own coarse channel — the paper's own
+partition, no data-path collective — weak scaling.
+
+--impl reference times the float64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "realtime_1.28MHz_coarse_channels_per_gpu_512_inputs"
+UNIT = "coarse channels sustained in real time (whole job)"
+SAMPLE_RATE = 1.28e6
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return {"hbm_gbs": p["hbm_gbs"], "tensor_burst": p["bf16_tflops"], "tensor_sustained": p["bf16_tflops_sustained"],
+                "source": "measured"}
+    return {"hbm_gbs": 6650.0, "tensor_burst": 1590.0, "tensor_sustained": 1400.0, "source": "fallback"}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period: float = 0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksEventReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksEventReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksEventReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksEventReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(s)}
+
+
+def physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[local_rank])
+        except Exception:
+            return local_rank
+    return local_rank
+
+
+def run_reference(args):
+    """The oracle, as it stands, on the host cores: a bounded sample of the workload per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import numpy as np
+    from oracle import oracle
+    from paper_2303_11557_b200 import synth
+    cfg = synth.CONFIGS[args.workload]
+    N, K, F = cfg.n_fft, cfg.n_keep, cfg.f_avg
+    # sample: all inputs, all channels, the first t_s spectra of dump 0 (t_s chosen for ~5-10 s per step)
+    t_s = 24 if args.workload == "C3" else 1
+    spec = cfg.spec()
+    spec.n_samples = t_s * N
+    volt = synth.gauss_voltages(spec)
+    oracle.build()
+    times = []
+    for it in range(args.warmup + args.steps):
+        t0 = time.perf_counter()
+        oracle.fx(volt, N, K, t_s, F)
+        t1 = time.perf_counter()
+        if it >= args.warmup:
+            times.append(t1 - t0)
+    sec = sum(times) / len(times)
+    data_seconds = t_s * N / SAMPLE_RATE
+    value = data_seconds / sec
+    sample = f"all {cfg.n_inputs} inputs, all {K} fine channels, first {t_s} spectra ({data_seconds*1e3:.2f} ms of data) of dump 0"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_fft": N, "n_keep": K, "f_avg": F,
+                       "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def cpu_baseline(cfg, budget_spectra):
+    import numpy as np
+    from oracle import oracle
+    from paper_2303_11557_b200 import synth
+    oracle.build()
+    N, K, F = cfg.n_fft, cfg.n_keep, cfg.f_avg
+    spec = cfg.spec()
+    spec.n_samples = budget_spectra * N
+    volt = synth.gauss_voltages(spec)
+    t0 = time.perf_counter()
+    oracle.fx(volt, N, K, budget_spectra, F)
+    sec = time.perf_counter() - t0
+    data_seconds = budget_spectra * N / SAMPLE_RATE
+    return {"value": data_seconds / sec, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"all {cfg.n_inputs} inputs, all {K} fine channels, first {budget_spectra} spectra "
+                      f"({data_seconds*1e3:.2f} ms of data) in {sec:.1f} s",
+            "seconds": sec}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C3", "C4"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 0)
+
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2303_11557_b200 import corr, synth
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cfg = synth.CONFIGS[args.workload]
+    n, N, K, T, F, D = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg, cfg.n_dumps
+    B = n * (n + 1) // 2
+    C = K // F
+    row = cfg.samples_per_input
+    data_seconds = cfg.seconds_of_data
+
+    # seeded synthetic voltages, one coarse channel per rank (coarse index = rank), resident in HBM
+    host = torch.empty((1, n, row, 2), dtype=torch.int8).pin_memory()
+    synth.gauss_voltages(cfg.spec(coarse=rank), out=host.numpy()[0])
+    volt = host.cuda()
+    h = corr.MwaxCorr(n, N, K, T, F)
+    vis = h.new_output(n_dumps=D)
+    stream = torch.cuda.current_stream()
+    dump_bytes = T * N * 2
+
+    def step(events=None):
+        for d in range(D):
+            v = volt[0, :, d * T * N:, :]
+            ptr_off = d * dump_bytes
+            if events is not None:
+                e0, e1, e2 = events[d]
+                e0.record(stream)
+            corr._check(corr.lib().mwax_corr_f_stage(h._h, volt.data_ptr() + ptr_off, row, int(stream.cuda_stream)), "f_stage", h._h)
+            if events is not None:
+                e1.record(stream)
+            corr._check(corr.lib().mwax_corr_x_stage(h._h, vis[0, d].data_ptr(), int(stream.cuda_stream)), "x_stage", h._h)
+            if events is not None:
+                e2.record(stream)
+
+    for _ in range(args.warmup):
+        step()
+    torch.cuda.synchronize()
+
+    evs = [[tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(D)] for _ in range(args.steps)]
+    sampler = ClockSampler(physical_gpu_index(local_rank))
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    t_start = torch.cuda.Event(enable_timing=True)
+    t_end = torch.cuda.Event(enable_timing=True)
+    t_start.record(stream)
+    for k in range(args.steps):
+        step(evs[k])
+    t_end.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop()
+    total_ms = t_start.elapsed_time(t_end)
+    if world > 1:
+        tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    f_ms = [e[0].elapsed_time(e[1]) for s in evs for e in s]
+    x_ms = [e[1].elapsed_time(e[2]) for s in evs for e in s]
+    f_avg_ms, x_avg_ms = sum(f_ms) / len(f_ms), sum(x_ms) / len(x_ms)
+    value = world * data_seconds / (ms_per_step * 1e-3)
+
+    # ---- e2e through the public host-buffer call (H2D + D2H inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        hvis = torch.empty((1, D, C, B, 2), dtype=torch.float32).pin_memory()
+        e_steps = max(2, min(args.steps, 5))
+        h.process_host(host, hvis, D, 1)          # warm-up (allocates staging)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(e_steps):
+            h.process_host(host, hvis, D, 1)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        e_ms = e0.elapsed_time(e1) / e_steps
+        if world > 1:
+            tt = torch.tensor([e_ms], device="cuda", dtype=torch.float64)
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            e_ms = float(tt.item())
+        e2e = {"value": world * data_seconds / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.numel(),
+               "d2h_bytes_per_step": hvis.numel() * 4, "ms_per_step": e_ms, "steps": e_steps}
+
+    if rank == 0:
+        peaks = load_peaks()
+        timed_s = total_ms * 1e-3
+        peak_kind = "sustained" if timed_s >= 1.0 else "burst"
+        tensor_peak = peaks["tensor_sustained"] if peak_kind == "sustained" else peaks["tensor_burst"]
+        # dominant kernel: X stage.  Algorithmic flops: 8 * n(n+1)/2 per (fine channel, time) sample
+        x_flops = 8.0 * B * K * T
+        x_ach = x_flops / (x_avg_ms * 1e-3) / 1e12
+        f_bytes = n * T * N * 2.0 + n * T * K * 4.0          # 2 B in + 4 B out per kept sample
+        f_ach = f_bytes / (f_avg_ms * 1e-3) / 1e9
+        x_dom = x_avg_ms >= f_avg_ms
+        roof_x = {"kernel": "x_stage_kernel<fp16>", "bound": "tensor", "achieved": x_ach, "peak": tensor_peak,
+                  "unit": "TFLOP/s", "frac": x_ach / tensor_peak, "traffic": None, "avg_launch_ms": x_avg_ms,
+                  "peak_source": f"{peaks['source']} bf16 {peak_kind} (MEASURED_PEAKS.json)",
+                  "frac_of_nominal_2250": x_ach / 2250.0}
+        roof_f = {"kernel": "f_stage_kernel", "bound": "hbm", "achieved": f_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                  "frac": f_ach / peaks["hbm_gbs"], "traffic": None, "avg_launch_ms": f_avg_ms,
+                  "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)"}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f16 operands, f32 accumulate (FFT in f32)", "data": "synthetic",
+                "config": {"workload": cfg.name, "n_inputs": n, "n_fft": N, "n_keep": K, "t_int": T, "f_avg": F,
+                           "dumps_per_step": D, "seconds_of_data_per_step": data_seconds,
+                           "coarse_channels_per_gpu_per_step": 1, "parallelism": f"coarse-channel x{world}",
+                           "l2": "inputs larger than L2 (%.2f GB in, %.2f GB workspace per dump)" %
+                                 (host.numel() / 1e9, h.workspace_bytes() / 1e9)},
+                "input_samples_per_s": world * n * row / (ms_per_step * 1e-3),
+                "gpu_launches": args.steps * D * h.launches_per_process(),
+                "clocks": clocks,
+                "roofline": roof_x if x_dom else roof_f,
+                "stages": {"f": roof_f, "x": roof_x},
+                "paper_context": "MWAX on 1 x A40 + 2 x Epyc 7F72: 5.9 s per 8 s subfile at 256 tiles, 1 s/10 kHz mode "
+                                 "=> 1 coarse channel per GPU in real time (PAPER.md Table 2 L531-545)"}
+        if e2e is not None:
+            line["e2e"] = e2e
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline(cfg, 24 if args.workload == "C3" else 1)
+        print(json.dumps(line), flush=True)
+    h.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -24,7 +24,9 @@ struct FParams {
     int radix[16];
     int vec_ok;              // 16-byte loads allowed
     const float2 *tw;        // [N] exp(-2 pi i m / N)
-    const float *sw;         // [K] per-position factor: s * sqrt(w_p)
+    const float *sw;         // [K] per-position factor sqrt(w_p): 1, sqrt(1/2) on a shared edge, 0 for excluded DC
+    float in_scale;          // s: power-of-two F-stage scale (keeps fp16 in range)
+    int chan_scale;          // 0 when every sw[p] == 1
     __half2 *Y;              // [K][T][pitch2]
     int pitch2;              // half2 (complex) elements per Y row
 };
@@ -162,7 +164,7 @@ __global__ void __launch_bounds__(256) f_stage_generic_kernel(const FParams P)
         if (i >= P.n_inputs) continue;
         int k = p - half;
         if (k < 0) k += N;
-        const float f = __ldg(&P.sw[p]);
+        const float f = __ldg(&P.sw[p]) * P.in_scale;
         const float2 v = src[k * G + g];
         P.Y[((long long)p * P.T + t) * P.pitch2 + i] = __floats2half2_rn(v.x * f, v.y * f);
     }

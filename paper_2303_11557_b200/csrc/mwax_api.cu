@@ -14,6 +14,7 @@
 
 #include "../../include/mwax_corr.h"
 #include "f_stage.cuh"
+#include "f_stage_pow2.cuh"
 #include "x_stage.cuh"
 
 namespace {
@@ -97,6 +98,11 @@ int upload(T **dptr, const std::vector<T> &h)
     return MWAX_OK;
 }
 
+using F64 = mwax::FPow2Config<64, 8, 16>;
+using F128 = mwax::FPow2Config<128, 8, 16>;
+using F256 = mwax::FPow2Config<256, 16, 32>;
+using F512 = mwax::FPow2Config<512, 16, 32>;
+
 template <bool kInt8, int BN>
 int launch_x(const CUtensorMap &tmap, const mwax::XParams &xp, int sm_count, cudaStream_t st)
 {
@@ -127,6 +133,9 @@ struct mwax_corr {
     int last_cuda;
     bool tables_ready;
     // F plan
+    int f_kind;        // 0 = generic Stockham kernel, else the power-of-two register kernel for that N
+    float in_scale;
+    int chan_scale;
     int G;
     size_t f_smem;
     std::vector<int> radix;
@@ -177,7 +186,7 @@ static void free_tables(mwax_corr *h)
 
 // Averaging geometry -> per-position factor sw[p], per-channel first tap and epilogue scale.
 // The weights of PAPER.md L290-298 are folded as  W[c][p] = scale_c * s^2-normalised sw[p]^2 :
-//   sw[p]   = s * sqrt(w_p), w_p = 1 inside a group, 1/2 on a shared edge (even F), 0 for the DC fine channel (F > 1)
+//   sw[p]   = sqrt(w_p) (the F stage also applies the power-of-two scale s), w_p = 1 inside a group, 1/2 on a shared edge (even F), 0 for the DC fine channel (F > 1)
 //   scale_c = 1/(s^2 F), times F/(F-1) for the centre channel when F > 1.
 static int build_tables(mwax_corr *h)
 {
@@ -185,7 +194,9 @@ static int build_tables(mwax_corr *h)
     const int K = h->K, F = h->F, C = h->C;
     const int lg = (int)std::ceil(std::log2((double)h->N) / 2.0);
     const double s = std::ldexp(1.0, -lg);   // power of two near 1/sqrt(N): keeps fp16 in range, epilogue exact
-    std::vector<float> sw(K, (float)s), scale(C, (float)(1.0 / (s * s * F)));
+    h->in_scale = (float)s;
+    h->chan_scale = 0;
+    std::vector<float> sw(K, 1.0f), scale(C, (float)(1.0 / (s * s * F)));
     std::vector<int> tap(C);
     if (h->avg_mode == MWAX_AVG_BLOCK || F == 1) {
         h->n_taps = F;
@@ -201,9 +212,10 @@ static int build_tables(mwax_corr *h)
         if (F % 2 == 0)
             for (int p = 0; p < K; ++p) {
                 const int u = p - half;
-                if ((((u - F / 2) % F) + F) % F == 0) sw[p] = (float)(s * std::sqrt(0.5));
+                if ((((u - F / 2) % F) + F) % F == 0) sw[p] = (float)std::sqrt(0.5);
             }
         sw[half] = 0.0f;                                            // DC excluded (L290-294)
+        h->chan_scale = 1;
         scale[c0] = (float)((1.0 / (s * s * F)) * (double)F / (double)(F - 1));
     }
     std::vector<uint8_t> tiles;
@@ -259,15 +271,29 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     h->sm_count = sm;
     h->last_cuda = 0;
     h->radix = radix;
-    // F plan: as many adjacent inputs per CTA as fit (two fp32 ping-pong buffers), up to 32 (128-byte segments)
+    // F plan: register two-pass kernel for N in {64,128,256,512}; otherwise the generic Stockham kernel with as
+    // many adjacent inputs per CTA as fit (two fp32 ping-pong buffers), up to 32 (128-byte segments)
     int G = 32;
     while (G > 1 && (size_t)2 * G * n_fft * sizeof(float2) > 200 * 1024) G >>= 1;
     h->G = G;
     h->f_smem = (size_t)2 * G * n_fft * sizeof(float2);
-    if (cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)h->f_smem) != cudaSuccess) {
-        g_last_error = MWAX_ERR_CUDA; delete h; return nullptr;
+    h->f_kind = 0;
+    if (const char *e = getenv("MWAX_F_GENERIC")) { if (atoi(e) == 1) n_fft = -n_fft; }
+    cudaError_t ae = cudaSuccess;
+    switch (n_fft) {
+        case 64: h->f_kind = 64; h->f_smem = F64::SMEM_BYTES;
+            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<64, 8, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64::SMEM_BYTES); break;
+        case 128: h->f_kind = 128; h->f_smem = F128::SMEM_BYTES;
+            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<128, 8, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, F128::SMEM_BYTES); break;
+        case 256: h->f_kind = 256; h->f_smem = F256::SMEM_BYTES;
+            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<256, 16, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, F256::SMEM_BYTES); break;
+        case 512: h->f_kind = 512; h->f_smem = F512::SMEM_BYTES;
+            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<512, 16, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, F512::SMEM_BYTES); break;
+        default:
+            ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
     }
+    if (n_fft < 0) n_fft = -n_fft;
+    if (ae != cudaSuccess) { g_last_error = MWAX_ERR_CUDA; delete h; return nullptr; }
     // twiddles exp(-2 pi i m / N), computed in double
     std::vector<float2> tw(n_fft);
     for (int m = 0; m < n_fft; ++m) {
@@ -311,10 +337,21 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
     fp.n_pass = (int)h->radix.size();
     for (int i = 0; i < fp.n_pass; ++i) fp.radix[i] = h->radix[i];
     fp.vec_ok = (h->N % 8 == 0) && (row_pitch % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_volt) & 15u) == 0);
-    fp.tw = h->d_tw; fp.sw = h->d_sw;
+    fp.tw = h->d_tw; fp.sw = h->d_sw; fp.in_scale = h->in_scale; fp.chan_scale = h->chan_scale;
     fp.Y = reinterpret_cast<__half2 *>(h->d_Y); fp.pitch2 = h->pitch / 2;
-    dim3 grid((h->n + h->G - 1) / h->G, h->T);
-    mwax::f_stage_generic_kernel<<<grid, 256, h->f_smem, (cudaStream_t)stream>>>(fp);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (h->f_kind) {
+        dim3 grid((h->n + 31) / 32, h->T);
+        switch (h->f_kind) {
+            case 64: mwax::f_stage_pow2_kernel<64, 8, 16><<<grid, F64::THREADS, F64::SMEM_BYTES, st>>>(fp); break;
+            case 128: mwax::f_stage_pow2_kernel<128, 8, 16><<<grid, F128::THREADS, F128::SMEM_BYTES, st>>>(fp); break;
+            case 256: mwax::f_stage_pow2_kernel<256, 16, 32><<<grid, F256::THREADS, F256::SMEM_BYTES, st>>>(fp); break;
+            default: mwax::f_stage_pow2_kernel<512, 16, 32><<<grid, F512::THREADS, F512::SMEM_BYTES, st>>>(fp); break;
+        }
+    } else {
+        dim3 grid((h->n + h->G - 1) / h->G, h->T);
+        mwax::f_stage_generic_kernel<<<grid, 256, h->f_smem, st>>>(fp);
+    }
     return note_cuda(&h->last_cuda);
 }
 

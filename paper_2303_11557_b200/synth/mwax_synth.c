@@ -14,6 +14,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <stddef.h>
+#include <stdlib.h>
 
 #define SYNTH_STREAM_NOISE  1u   /* g_i[m]  : independent per input             */
 #define SYNTH_STREAM_COMMON 2u   /* s[m]    : shared by all inputs of a coarse  */
@@ -70,32 +71,60 @@ void mwax_synth_gauss(uint64_t seed, uint32_t coarse,
 {
     const double two_pi = 6.283185307179586476925286766559;
     const double a_noise = sqrt(1.0 - rho) * sigma, a_common = sqrt(rho) * sigma;
-#pragma omp parallel for collapse(2) schedule(static)
-    for (int ii = 0; ii < n_gen; ++ii) {
-        for (int64_t blk = 0; blk < (n_samples + 4095) / 4096; ++blk) {
+    const int use_common = (rho != 0.0);
+    /* the common signal s[m] is the same for every input: draw it once */
+    double *cs = NULL;
+    if (use_common) {
+        cs = (double *)malloc(sizeof(double) * 2 * (size_t)n_samples);
+        if (!cs) return;
+#pragma omp parallel for schedule(static)
+        for (int64_t mm = 0; mm < n_samples; ++mm)
+            normal_pair(draw(seed, SYNTH_STREAM_COMMON, coarse, 0u, (uint64_t)(sample0 + mm)), &cs[2 * mm], &cs[2 * mm + 1]);
+    }
+#pragma omp parallel
+    {
+        /* per-input tone sum over one frame (tones are on integer bins, so they repeat every tone_nfft samples) */
+        double *tt = (n_tones > 0) ? (double *)malloc(sizeof(double) * 2 * (size_t)tone_nfft) : NULL;
+#pragma omp for schedule(dynamic, 1)
+        for (int ii = 0; ii < n_gen; ++ii) {
             const int i = input0 + ii;
-            int64_t m_end = (blk + 1) * 4096 < n_samples ? (blk + 1) * 4096 : n_samples;
-            for (int64_t mm = blk * 4096; mm < m_end; ++mm) {
+            if (tt) {
+                for (int r = 0; r < tone_nfft; ++r) {
+                    double re = 0.0, im = 0.0;
+                    for (int k = 0; k < n_tones; ++k) {
+                        int64_t km = ((int64_t)tone_bin[k] * r) % tone_nfft;
+                        if (km < 0) km += tone_nfft;
+                        int64_t ph_i = ((int64_t)tone_phase_mult[k] * i) % n_total;
+                        double ph = two_pi * ((double)km / (double)tone_nfft + (double)ph_i / (double)n_total);
+                        re += tone_amp[k] * cos(ph);
+                        im += tone_amp[k] * sin(ph);
+                    }
+                    tt[2 * r] = re;
+                    tt[2 * r + 1] = im;
+                }
+            }
+            for (int64_t mm = 0; mm < n_samples; ++mm) {
                 const int64_t m = sample0 + mm;
-                double gr, gi, sr, si;
+                double gr, gi;
                 normal_pair(draw(seed, SYNTH_STREAM_NOISE, coarse, (uint32_t)i, (uint64_t)m), &gr, &gi);
-                normal_pair(draw(seed, SYNTH_STREAM_COMMON, coarse, 0u, (uint64_t)m), &sr, &si);
-                double re = a_noise * gr + a_common * sr;
-                double im = a_noise * gi + a_common * si;
-                for (int k = 0; k < n_tones; ++k) {
-                    int64_t km = ((int64_t)tone_bin[k] * (m % tone_nfft)) % tone_nfft;
-                    if (km < 0) km += tone_nfft;
-                    int64_t ph_i = ((int64_t)tone_phase_mult[k] * i) % n_total;
-                    double ph = two_pi * ((double)km / (double)tone_nfft + (double)ph_i / (double)n_total);
-                    re += tone_amp[k] * cos(ph);
-                    im += tone_amp[k] * sin(ph);
+                double re = a_noise * gr, im = a_noise * gi;
+                if (use_common) {
+                    re += a_common * cs[2 * mm];
+                    im += a_common * cs[2 * mm + 1];
+                }
+                if (tt) {
+                    const int r = (int)(m % tone_nfft);
+                    re += tt[2 * r];
+                    im += tt[2 * r + 1];
                 }
                 int8_t *o = out + 2 * ((int64_t)ii * row_pitch + mm);
                 o[0] = clip_round(re, 127);
                 o[1] = clip_round(im, 127);
             }
         }
+        free(tt);
     }
+    free(cs);
 }
 
 /*

@@ -1,0 +1,266 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle on the same seeded inputs.
+
+Bars (BASELINE.json north star): int8 X-only path bit-exact; float path |V_gpu - V_ref| <= 2e-3 * sqrt(A_i A_j) per
+visibility, A = the oracle's autocorrelation in the same (dump, channel); no absolute floor (all-zero data must
+give exact zeros).  Small cases are compared element by element; BASELINE.json's full-size configs are compared
+on sampled inputs (every pair among a selection that straddles the tile boundaries) which the oracle computes
+one by one, in the launch configuration bench.py times.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import oracle
+from paper_2303_11557_b200 import corr, synth
+
+pytestmark = pytest.mark.gpu
+
+TOL = 2e-3   # north star: |V_gpu - V_ref| <= 2e-3 sqrt(A_i A_j)
+
+
+def _complex(vis_f32):
+    v = vis_f32.astype(np.float64)
+    return v[..., 0] + 1j * v[..., 1]
+
+
+def _norm_err(got, ref, n_sel):
+    """got, ref complex [C][B_sel] over the same selection; returns max |got-ref| / sqrt(A_i A_j)."""
+    A = np.array([ref[:, oracle.baseline_index(i, i)].real for i in range(n_sel)])     # [n_sel][C]
+    ii, jj = np.tril_indices(n_sel)
+    norm = np.sqrt(A[ii] * A[jj]).T
+    d = np.abs(got - ref)
+    assert np.all(d[norm == 0] == 0), "non-zero output where the oracle's autocorrelations vanish"
+    with np.errstate(invalid="ignore", divide="ignore"):
+        e = np.where(norm > 0, d / norm, 0.0)
+    return float(e.max())
+
+
+def _gather_sel(full, sel):
+    """full [..., B_full] -> [..., B_sel] for sorted selection sel (pairs (a >= b) -> inputs (sel[a], sel[b]))."""
+    sel = np.asarray(sel)
+    a, b = np.tril_indices(len(sel))
+    idx = sel[a] * (sel[a] + 1) // 2 + sel[b]
+    return full[..., idx]
+
+
+def _run_fx(volt, n, N, K, T, F, mode=0, n_dumps=1):
+    h = corr.MwaxCorr(n, N, K, T, F, avg_mode=mode)
+    v = torch.from_numpy(volt).cuda()
+    out = h.new_output(n_dumps=n_dumps)
+    out.fill_(float("nan"))
+    if n_dumps == 1 and volt.shape[1] == T * N:
+        h.process(v, out[0, 0])
+    else:
+        h.process_batch(v[None], out, n_dumps)
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy()[0])
+    h.destroy()
+    return got     # [D][C][B]
+
+
+# ---------------------------------------------------------------------------------------------- int8 X-only
+@pytest.mark.parametrize("n,n_chan,n_time", [
+    (8, 1, 1), (8, 2, 31), (16, 3, 128), (64, 2, 129), (72, 3, 300), (136, 2, 257), (200, 5, 1000), (512, 2, 2000),
+])
+def test_int8_bit_exact_elementwise(n, n_chan, n_time):
+    z = synth.uniform_voltages(n_chan, n_time, n, n_shared=min(64, n), seed=100 + n)
+    h = corr.MwaxXcorrI8(n, n_chan, n_time)
+    out = h.new_output()
+    out.fill_(-12345)
+    h.process(torch.from_numpy(z).cuda(), out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oracle.xcorr_i8(z))
+    h.destroy()
+
+
+def test_int8_extreme_values_bit_exact():
+    """-128 and +127 everywhere it hurts: accumulator magnitude 2*128^2*T stays exact in int32."""
+    n, n_chan, n_time = 24, 2, 4000
+    rng = np.random.default_rng(5)
+    z = rng.choice(np.array([-128, -127, 127, 0, 1], dtype=np.int8), size=(n_chan, n_time, n, 2))
+    z[0, :, 0, :] = -128
+    z[0, :, 1, :] = 127
+    h = corr.MwaxXcorrI8(n, n_chan, n_time)
+    out = h.new_output()
+    h.process(torch.from_numpy(z).cuda(), out)
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oracle.xcorr_i8(z))
+    h.destroy()
+
+
+def test_int8_config2_full_size_sampled():
+    """BASELINE.json configs[1]: 512 inputs x 1024 channels x 2000 samples; the oracle computes every pair among
+    a selection of inputs straddling all tile boundaries, for every channel."""
+    n, n_chan, n_time = 512, 1024, 2000
+    z = synth.uniform_voltages(n_chan, n_time, n)          # recipe: U{-8..7} + shared component on inputs 0-63
+    h = corr.MwaxXcorrI8(n, n_chan, n_time)
+    out = h.new_output()
+    h.process(torch.from_numpy(z).cuda(), out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    sel = np.array([0, 1, 31, 63, 64, 65, 127, 128, 129, 191, 255, 256, 300, 383, 384, 448, 510, 511])
+    ref = oracle.xcorr_i8(z, sel=sel)
+    a, b = np.tril_indices(len(sel))
+    idx = sel[a] * (sel[a] + 1) // 2 + sel[b]
+    assert np.array_equal(got[:, idx, :], ref)
+    # properties that hold at any size: autos real, non-negative, equal to the summed power
+    ii = np.arange(n)
+    autos = got[:, ii * (ii + 1) // 2 + ii, :]
+    assert np.all(autos[..., 1] == 0) and np.all(autos[..., 0] >= 0)
+    power = (z.astype(np.int64) ** 2).sum(axis=(1, 3))      # [chan][input]
+    assert np.array_equal(autos[..., 0].astype(np.int64), power)
+    h.destroy()
+
+
+# ---------------------------------------------------------------------------------------------- float FX path
+def test_config1_tiny_fx_elementwise():
+    """BASELINE.json configs[0]: 16 inputs, N = K = 64, 256 spectra, rho = 0.3, tone at bin +5."""
+    cfg = synth.CONFIGS["C1"]
+    volt = synth.gauss_voltages(cfg.spec())
+    ref = oracle.fx(volt, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg)
+    got = _run_fx(volt, cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg)[0]
+    assert _norm_err(got, ref, cfg.n_inputs) <= TOL
+    # the tone lands at position 5 + 32 with phase 2 pi (i - j) / 16 (reading Q18)
+    p = 37
+    n = cfg.n_inputs
+    auto = np.array([got[:, oracle.baseline_index(i, i)].real for i in range(n)])
+    assert np.all(auto.argmax(axis=1) == p)
+    v = got[p, oracle.baseline_index(9, 4)]
+    assert abs(np.angle(v * np.exp(-2j * np.pi * (9 - 4) / 16))) < 0.05
+
+
+@pytest.mark.parametrize("n,N,K,T,F,mode", [
+    (1, 64, 64, 8, 1, 0),          # a single input: one auto per channel
+    (3, 5, 5, 7, 1, 0),            # tiny odd everything, scalar-load path
+    (16, 64, 64, 40, 2, 0),        # even F: F+1 taps, half-weight edges, cyclic wrap of channel 0
+    (16, 64, 64, 40, 2, 1),        # BLOCK mode
+    (24, 100, 50, 33, 5, 0),       # radix-5, K < N, odd F, DC exclusion
+    (40, 250, 250, 17, 25, 0),     # 2 * 5^3
+    (70, 128, 96, 65, 4, 0),       # ragged inputs (pad columns), T one past a 64-row block
+    (130, 128, 128, 100, 1, 0),    # inputs straddle a 128-input tile
+    (200, 256, 256, 20, 2, 0),     # config-5 shape cut down
+    (33, 512, 512, 9, 4, 0),       # largest register-kernel length
+    (33, 64, 48, 9, 1, 0),         # keep < fft in the register kernel
+    (40, 2048, 2048, 3, 1, 0),     # power of two beyond the register kernel (generic Stockham path)
+    (12, 1024, 1000, 6, 8, 0),
+    (8, 6400, 6400, 4, 50, 0),     # the paper's mode, cut down
+    (8, 6400, 6400, 3, 256, 0),    # odd number of output channels (25)
+    (20, 6400, 6400, 2, 1, 0),     # no averaging at N = 6400
+])
+def test_fx_elementwise_shapes(n, N, K, T, F, mode):
+    tones = [synth.Tone(min(3, K // 2 - 1), 6.0, 1)] if K > 8 else []
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=tones, seed=1000 + n + N)
+    volt = synth.gauss_voltages(spec)
+    ref = oracle.fx(volt, N, K, T, F, mode)
+    got = _run_fx(volt, n, N, K, T, F, mode)[0]
+    assert not np.isnan(got.view(np.float64)).any()
+    assert _norm_err(got, ref, n) <= TOL
+    ii = np.arange(n)
+    autos = got[:, ii * (ii + 1) // 2 + ii]
+    assert np.all(autos.imag == 0.0) and np.all(autos.real >= 0.0)
+
+
+def test_fx_all_zero_input_gives_exact_zeros():
+    n, N, T = 16, 64, 10
+    volt = np.zeros((n, N * T, 2), dtype=np.int8)
+    got = _run_fx(volt, n, N, N, T, 2)[0]
+    assert np.all(got == 0)
+
+
+def test_fx_full_scale_tone_does_not_overflow_fp16():
+    """+-127 full-scale tone at N = 6400: |X| = 127 sqrt(2) N would overflow fp16 without the F-stage scaling."""
+    n, N, T, F = 8, 6400, 2, 50
+    q = np.arange(N * T)
+    x = 127.0 * np.exp(2j * np.pi * ((1010 * q) % N) / N)
+    volt = np.empty((n, N * T, 2), dtype=np.int8)
+    volt[..., 0] = np.rint(x.real)
+    volt[..., 1] = np.rint(x.imag)
+    volt[3] = np.random.default_rng(3).choice(np.array([-128, 127], dtype=np.int8), size=(N * T, 2))
+    ref = oracle.fx(volt, N, N, T, F)
+    got = _run_fx(volt, n, N, N, T, F)[0]
+    assert np.isfinite(got.view(np.float64)).all()
+    assert _norm_err(got, ref, n) <= TOL
+
+
+def test_fx_additivity_over_dumps_and_batch_layout():
+    """process_batch with a row pitch longer than one integration: dump d uses samples [dTN, (d+1)TN) of every
+    row; an integration over 2T equals the sum of the two integrations over T."""
+    n, N, T = 48, 128, 30
+    spec = synth.GaussSpec(n, N * 2 * T, N, sigma=16.0, rho=0.1, seed=77)
+    volt = synth.gauss_voltages(spec)
+    two = _run_fx(volt, n, N, N, T, 1, n_dumps=2)
+    whole = _run_fx(volt, n, N, N, 2 * T, 1)[0]
+    ref0 = oracle.fx(volt, N, N, T, 1, dump=0)
+    ref1 = oracle.fx(volt, N, N, T, 1, dump=1)
+    assert _norm_err(two[0], ref0, n) <= TOL and _norm_err(two[1], ref1, n) <= TOL
+    assert _norm_err(two[0] + two[1], ref0 + ref1, n) <= TOL
+    assert _norm_err(whole, ref0 + ref1, n) <= TOL
+
+
+SEL = [0, 1, 62, 63, 64, 127, 128, 129, 255, 256, 383, 384, 510, 511]
+
+
+@pytest.mark.parametrize("name", ["C3", "C4"])
+def test_fx_full_size_configs_sampled(name):
+    """BASELINE.json configs[2]/[3] at full size through process_batch (the launch configuration bench.py times);
+    the oracle computes every pair among SEL (inputs on both sides of every 64/128-input tile edge), all channels,
+    both dumps."""
+    cfg = synth.CONFIGS[name]
+    n, N, K, T, F, D = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg, cfg.n_dumps
+    host = torch.empty((1, n, cfg.samples_per_input, 2), dtype=torch.int8)
+    volt = host.numpy()[0]
+    synth.gauss_voltages(cfg.spec(), out=volt)
+    h = corr.MwaxCorr(n, N, K, T, F)
+    out = h.new_output(n_dumps=D)
+    h.process_batch(host.cuda(), out, D)
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy()[0])
+    h.destroy()
+    for d in range(D):
+        ref = oracle.fx(volt, N, K, T, F, dump=d, sel=np.array(SEL))
+        assert _norm_err(_gather_sel(got[d], SEL), ref, len(SEL)) <= TOL
+    ii = np.arange(n)
+    autos = got[..., ii * (ii + 1) // 2 + ii]
+    assert np.all(autos.imag == 0.0) and np.all(autos.real >= 0.0)
+    if name == "C4":
+        # the DC tone (amplitude 10 on every input) must vanish from the centre output channel:
+        # that channel's autos stay at the noise level of its neighbours
+        c0 = (K // F) // 2
+        assert np.all(autos[:, c0] < 1.5 * autos[:, c0 + 1])
+
+
+def test_fx_config5_shape_two_coarse_channels_sampled():
+    """BASELINE.json configs[4] cut to 2 of its 8 coarse channels (same per-channel sizes: 1024 inputs, N = 256,
+    F = 2, 2 dumps of 1250 spectra), [coarse][input][time] layout through process_batch."""
+    cfg = synth.CONFIGS["C5"]
+    n, N, K, T, F, D = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg, cfg.n_dumps
+    n_coarse = 2
+    host = torch.empty((n_coarse, n, cfg.samples_per_input, 2), dtype=torch.int8)
+    for c in range(n_coarse):
+        synth.gauss_voltages(cfg.spec(coarse=c), out=host.numpy()[c])
+    h = corr.MwaxCorr(n, N, K, T, F)
+    out = h.new_output(n_dumps=D, n_coarse=n_coarse)
+    h.process_batch(host.cuda(), out, D, n_coarse)
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy())
+    h.destroy()
+    sel = [0, 63, 64, 127, 128, 511, 512, 767, 768, 1023]
+    for c in range(n_coarse):
+        for d in range(D):
+            ref = oracle.fx(host.numpy()[c], N, K, T, F, dump=d, sel=np.array(sel))
+            assert _norm_err(_gather_sel(got[c, d], sel), ref, len(sel)) <= TOL
+
+
+def test_host_buffer_entry_matches_device_entry():
+    n, N, T, D = 32, 128, 20, 2
+    spec = synth.GaussSpec(n, N * T * D, N, sigma=16.0, rho=0.1, seed=9)
+    volt = synth.gauss_voltages(spec)
+    h = corr.MwaxCorr(n, N, N, T, 2)
+    dev = h.new_output(n_dumps=D)
+    h.process_batch(torch.from_numpy(volt)[None].cuda(), dev, D)
+    hv = torch.from_numpy(volt)[None].contiguous().pin_memory()
+    hout = torch.empty(dev.shape, dtype=torch.float32).pin_memory()
+    h.process_host(hv, hout, D)
+    torch.cuda.synchronize()
+    assert torch.equal(hout, dev.cpu())
+    h.destroy()
