@@ -20,6 +20,7 @@ struct FParams {
     long long sample0;       // first sample of this dump in every row
     int n_inputs, N, K, T;
     int G;                   // inputs per CTA
+    int frames_per_cta;      // consecutive frames one CTA of the power-of-two kernel walks over
     int n_pass;
     int radix[16];
     int vec_ok;              // 16-byte loads allowed

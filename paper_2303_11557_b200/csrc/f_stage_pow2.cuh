@@ -1,7 +1,8 @@
-// f_stage_pow2.cuh — F stage for power-of-two frame lengths N = R1 * R2 in {64, 128, 256}: a register-resident
+// f_stage_pow2.cuh — F stage for power-of-two frame lengths N = R1 * R2 in {64, 128, 256, 512}: a register-resident
 // two-pass FFT in which LANE = INPUT.
 //
-// One CTA transforms one frame of 32 adjacent inputs.  Thread (warp w, lane L) works on input i0 + L only, so
+// One CTA owns 32 adjacent inputs and walks over a run of consecutive frames.  Thread (warp w, lane L) works on
+// input i0 + L only, so
 //   * every shared-memory exchange is [index][lane]: conflict free by construction;
 //   * every global store writes 32 adjacent inputs of one (channel, time) row: one full 128-byte line,
 //     i.e. the corner turn into Y[p][t][input] costs nothing (PAPER.md L274 did it as a separate pass).
@@ -9,6 +10,12 @@
 // twiddle W_N^{r k1}; exchange through shared memory; pass 2 (in registers): for its k1 the thread computes
 // X[k1 + R1 k2] = sum_r W_R2^{r k2} (W_N^{r k1} A_r[k1]).
 // int8 -> fp32 promotion happens in registers with the power-of-two F-stage scale folded in.
+//
+// The kernel is instruction-issue bound (ncu: profiles/r1_f128_*.md), so everything that is not butterfly
+// arithmetic is hoisted out of the frame loop: row pointers, the swizzle-free padded raw tile (row stride N/2+1
+// words -> bank = row + word), inter-pass twiddles read as broadcast 16-byte shared loads, and store addresses
+// formed as base + k2 * stride with compile-time k2.  The raw bytes of frame t+1 are fetched into registers while
+// frame t is being transformed.
 #pragma once
 #include <cuda_fp16.h>
 #include <cstdint>
@@ -89,116 +96,188 @@ struct FPow2Config {
     static constexpr int THREADS = 32 * W;
     static constexpr int RPT = PTS / R1;          // residues per thread in pass 1
     static constexpr int KPT = PTS / R2;          // k1 values per thread in pass 2
-    static constexpr int RAW_WORDS = 32 * (N / 2);          // 32 inputs x N samples x 2 bytes
-    static constexpr int SMEM_BYTES = RAW_WORDS * 4 + N * 32 * 8;
+    static constexpr int ROW_WORDS = N / 2 + 1;   // padded raw row: bank(row, word) = row + word (mod 32)
+    static constexpr int RAW_WORDS = 32 * ROW_WORDS;
+    static constexpr int TW_WORDS = 2 * N;        // inter-pass twiddles [r][k1] float2
+    static constexpr int EX_OFF_WORDS = ((RAW_WORDS + TW_WORDS + 3) / 4) * 4;
+    static constexpr int SMEM_BYTES = EX_OFF_WORDS * 4 + N * 32 * 8;
+    static constexpr int VPT = (32 * (N / 8)) / THREADS;   // 16-byte raw vectors per thread per frame
     static_assert(RPT >= 1 && KPT >= 1 && (RPT == 1 || RPT == 2), "unsupported split");
     static_assert(R1 * R2 == N && W * RPT == R2 && W * KPT == R1, "bad factorisation");
+    static_assert(VPT * THREADS == 32 * (N / 8), "raw tile must divide evenly over the threads");
+    static_assert(R1 % 4 == 0, "twiddle rows are read as 16-byte pairs");
 };
 
-template <int N, int R1, int PTS>
+// FULL : K == N (every bin is kept; no range checks)          SCALE : multiply by sw[p] (averaging weights)
+template <int N, int R1, int PTS, bool FULL, bool SCALE>
 __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2_kernel(const FParams P)
 {
     using C = FPow2Config<N, R1, PTS>;
     constexpr int R2 = C::R2;
-    extern __shared__ uint32_t fsm[];
-    uint32_t *raw = fsm;                                         // [32 rows][N/2 words], word index XOR lane
-    float2 *ex = reinterpret_cast<float2 *>(fsm + C::RAW_WORDS); // [k1][r][lane]
+    extern __shared__ __align__(16) uint32_t fsm[];
+    uint32_t *raw = fsm;                                              // [32 rows][ROW_WORDS]
+    float2 *twp = reinterpret_cast<float2 *>(fsm + C::RAW_WORDS + (C::RAW_WORDS & 1));   // [R2][R1] W_N^{r k1}
+    float2 *ex = reinterpret_cast<float2 *>(fsm + C::EX_OFF_WORDS);  // [k1][r][lane]
 
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i0 = blockIdx.x * 32;
-    const int t = blockIdx.y;
-    const long long s_off = P.sample0 + (long long)t * N;
+    const int t_begin = blockIdx.y * P.frames_per_cta;
+    const int t_end = min(P.T, t_begin + P.frames_per_cta);
 
-    // ---- coalesced 16-byte loads of the 32 rows (2N bytes each), scattered into raw with a per-row XOR swizzle
-    constexpr int VPR = N / 8;                                   // 16-byte vectors per row
-    for (int v = threadIdx.x; v < 32 * VPR; v += C::THREADS) {
-        const int row = v / VPR, c = v % VPR;
-        const int i = i0 + row;
-        int4 q = make_int4(0, 0, 0, 0);
-        if (i < P.n_inputs) {
-            const int8_t *src = P.volt + 2 * ((long long)i * P.row_pitch + s_off) + 16 * c;
-            if (P.vec_ok) {
-                q = __ldg(reinterpret_cast<const int4 *>(src));
-            } else {
-                const uint16_t *s16 = reinterpret_cast<const uint16_t *>(src);   // samples are 2-byte aligned
-                uint32_t ww[4];
+    // ---- per-CTA setup: twiddle rows, row pointers
+    for (int e = threadIdx.x; e < N; e += C::THREADS) {
+        const int r = e / R1, k1 = e % R1;
+        twp[e] = __ldg(&P.tw[r * k1]);
+    }
+    constexpr int VPR = N / 8;                                        // 16-byte vectors per row
+    const int8_t *src[C::VPT];
+    uint32_t *rdst[C::VPT];
+    bool rok[C::VPT];
 #pragma unroll
-                for (int e = 0; e < 4; ++e) ww[e] = (uint32_t)s16[2 * e] | ((uint32_t)s16[2 * e + 1] << 16);
-                q = make_int4((int)ww[0], (int)ww[1], (int)ww[2], (int)ww[3]);
+    for (int v = 0; v < C::VPT; ++v) {
+        const int idx = threadIdx.x + v * C::THREADS;
+        const int row = idx / VPR, c = idx % VPR;
+        rok[v] = (i0 + row) < P.n_inputs;
+        src[v] = P.volt + 2 * ((long long)(rok[v] ? i0 + row : 0) * P.row_pitch + P.sample0) + 16 * c;
+        rdst[v] = raw + row * C::ROW_WORDS + 4 * c;
+    }
+    auto fetch = [&](int t, int4 (&q)[C::VPT]) {
+#pragma unroll
+        for (int v = 0; v < C::VPT; ++v) {
+            q[v] = make_int4(0, 0, 0, 0);
+            if (rok[v]) {
+                const int8_t *s = src[v] + 2ll * t * N;
+                if (P.vec_ok) {
+                    q[v] = __ldg(reinterpret_cast<const int4 *>(s));
+                } else {
+                    const uint16_t *s16 = reinterpret_cast<const uint16_t *>(s);   // samples are 2-byte aligned
+                    uint32_t ww[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) ww[e] = (uint32_t)s16[2 * e] | ((uint32_t)s16[2 * e + 1] << 16);
+                    q[v] = make_int4((int)ww[0], (int)ww[1], (int)ww[2], (int)ww[3]);
+                }
             }
         }
-        uint32_t *dst = raw + row * (N / 2);
-        dst[(4 * c + 0) ^ row] = (uint32_t)q.x;
-        dst[(4 * c + 1) ^ row] = (uint32_t)q.y;
-        dst[(4 * c + 2) ^ row] = (uint32_t)q.z;
-        dst[(4 * c + 3) ^ row] = (uint32_t)q.w;
+    };
+    auto stash = [&](const int4 (&q)[C::VPT]) {
+#pragma unroll
+        for (int v = 0; v < C::VPT; ++v) {
+            rdst[v][0] = (uint32_t)q[v].x;
+            rdst[v][1] = (uint32_t)q[v].y;
+            rdst[v][2] = (uint32_t)q[v].z;
+            rdst[v][3] = (uint32_t)q[v].w;
+        }
+    };
+
+    int4 q[C::VPT];
+    if (t_begin < t_end) {
+        fetch(t_begin, q);
+        stash(q);
     }
     __syncthreads();
 
-    // ---- pass 1: this thread's residues r = w*RPT + e; points x[r + R2 j], j < R1
     // int8 -> fp32 with the F-stage scale s = 2^-sh folded in (exact): byte b -> ((b ^ 0x80) + 2^23 - (2^23 + 128)) * s
     const float s = P.in_scale;
     const float bias = -8388736.0f * s;
-    {
-        float2 x[C::RPT][R1];
-        const uint32_t *rrow = raw + lane * (N / 2);
-#pragma unroll
-        for (int j = 0; j < R1; ++j) {
-            if (C::RPT == 2) {
-                // samples q = 2w + R2 j and q + 1 share one 32-bit word
-                const uint32_t word = rrow[(w + (R2 / 2) * j) ^ lane] ^ 0x80808080u;
-                x[0][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), s, bias),
-                                      fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441)), s, bias));
-                x[C::RPT - 1][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7442)), s, bias),
-                                               fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7443)), s, bias));
-            } else {
-                const int q = w + R2 * j;
-                uint32_t word = rrow[(q >> 1) ^ lane] ^ 0x80808080u;
-                if (q & 1) word >>= 16;
-                x[0][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), s, bias),
-                                      fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441)), s, bias));
-            }
-        }
-#pragma unroll
-        for (int e = 0; e < C::RPT; ++e) {
-            fft_dif<R1>(x[e]);
-            const int r = w * C::RPT + e;
-#pragma unroll
-            for (int k1 = 0; k1 < R1; ++k1) {
-                float2 v = x[e][bitrev(k1, ilog2(R1))];
-                if (k1 > 0) v = cmul(v, __ldg(&P.tw[r * k1]));           // W_N^{r k1}; warp-uniform address
-                ex[(k1 * R2 + r) * 32 + lane] = v;
-            }
-        }
-    }
-    __syncthreads();
+    const uint32_t *rrow = raw + lane * C::ROW_WORDS + (C::RPT == 2 ? w : (w >> 1));
+    float2 *ex_w = ex + (w * C::RPT) * 32 + lane;                     // + (k1 * R2 + e) * 32
+    const float2 *ex_r = ex + (w * C::KPT) * R2 * 32 + lane;          // + (e * R2 + r) * 32
+    const float4 *tw_row = reinterpret_cast<const float4 *>(twp + (w * C::RPT) * R1);
 
-    // ---- pass 2: this thread's k1 = w*KPT + e; X[k1 + R1 k2] = FFT_R2 over r
+    // output addressing: position p of bin k = k1 + R1 k2 is k +- N/2 when K == N
     const int i = i0 + lane;
+    const bool iok = i < P.n_inputs;
     const int half = P.K / 2;
+    const size_t chan_stride = (size_t)P.T * P.pitch2;                // half2 elements between positions
+    __half2 *ybase = P.Y + i;
+
+    for (int t = t_begin; t < t_end; ++t) {
+        const bool more = (t + 1) < t_end;
+        if (more) fetch(t + 1, q);                                    // in flight during both passes
+
+        // ---- pass 1: this thread's residues r = w*RPT + e; points x[r + R2 j], j < R1
+        {
+            float2 x[C::RPT][R1];
 #pragma unroll
-    for (int e = 0; e < C::KPT; ++e) {
-        const int k1 = w * C::KPT + e;
-        float2 y[R2];
-#pragma unroll
-        for (int r = 0; r < R2; ++r) y[r] = ex[(k1 * R2 + r) * 32 + lane];
-        fft_dif<R2>(y);
-        if (i < P.n_inputs) {
-#pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) {
-                const int k = k1 + R1 * k2;
-                const int u = (k < N / 2) ? k : k - N;                   // signed bin
-                const int p = u + half;                                  // centre order
-                if (p < 0 || p >= P.K) continue;                         // keep the central K channels (L611)
-                float2 v = y[bitrev(k2, ilog2(R2))];
-                if (P.chan_scale) {
-                    const float f = __ldg(&P.sw[p]);                     // sqrt(w_p): shared edge / DC exclusion
-                    v.x *= f;
-                    v.y *= f;
+            for (int j = 0; j < R1; ++j) {
+                if (C::RPT == 2) {
+                    // samples q = 2w + R2 j and q + 1 share one 32-bit word
+                    const uint32_t word = rrow[(R2 / 2) * j] ^ 0x80808080u;
+                    x[0][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), s, bias),
+                                          fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441)), s, bias));
+                    x[C::RPT - 1][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7442)), s, bias),
+                                                   fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7443)), s, bias));
+                } else {
+                    uint32_t word = rrow[(R2 / 2) * j] ^ 0x80808080u;
+                    if (w & 1) word >>= 16;
+                    x[0][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), s, bias),
+                                          fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441)), s, bias));
                 }
-                P.Y[((long long)p * P.T + t) * P.pitch2 + i] = __floats2half2_rn(v.x, v.y);
+            }
+#pragma unroll
+            for (int e = 0; e < C::RPT; ++e) {
+                fft_dif<R1>(x[e]);
+#pragma unroll
+                for (int kk = 0; kk < R1; kk += 2) {
+                    const float4 tw2 = tw_row[(e * R1 + kk) / 2];     // W_N^{r kk}, W_N^{r (kk+1)}: warp-uniform
+                    float2 v0 = x[e][bitrev(kk, ilog2(R1))];
+                    float2 v1 = x[e][bitrev(kk + 1, ilog2(R1))];
+                    if (kk > 0) v0 = cmul(v0, make_float2(tw2.x, tw2.y));
+                    v1 = cmul(v1, make_float2(tw2.z, tw2.w));
+                    ex_w[(kk * R2 + e) * 32] = v0;
+                    ex_w[((kk + 1) * R2 + e) * 32] = v1;
+                }
             }
         }
+        __syncthreads();                                              // ex complete; raw(t) no longer needed
+        if (more) stash(q);
+
+        // ---- pass 2: this thread's k1 = w*KPT + e; X[k1 + R1 k2] = FFT_R2 over r
+#pragma unroll
+        for (int e = 0; e < C::KPT; ++e) {
+            const int k1 = w * C::KPT + e;
+            float2 y[R2];
+#pragma unroll
+            for (int r = 0; r < R2; ++r) y[r] = ex_r[(e * R2 + r) * 32];
+            fft_dif<R2>(y);
+            if (FULL) {
+                // k < N/2  <=>  k2 < R2/2:  p = k + N/2, else p = k - N/2
+                __half2 *yp = ybase + ((size_t)(k1 + N / 2) * P.T + t) * P.pitch2;
+                __half2 *yn = ybase + ((size_t)k1 * P.T + t) * P.pitch2;
+                const float *swp = P.sw + k1;
+                if (iok) {
+#pragma unroll
+                    for (int k2 = 0; k2 < R2; ++k2) {
+                        float2 v = y[bitrev(k2, ilog2(R2))];
+                        const int pk = (k2 < R2 / 2) ? (N / 2 + R1 * k2) : (R1 * k2 - N / 2);   // p - k1
+                        if (SCALE) {
+                            const float f = __ldg(swp + pk);
+                            v.x *= f;
+                            v.y *= f;
+                        }
+                        __half2 *dst = (k2 < R2 / 2) ? yp + (size_t)(R1 * k2) * chan_stride
+                                                     : yn + (size_t)(R1 * (k2 - R2 / 2)) * chan_stride;
+                        *dst = __floats2half2_rn(v.x, v.y);
+                    }
+                }
+            } else if (iok) {
+#pragma unroll
+                for (int k2 = 0; k2 < R2; ++k2) {
+                    const int k = k1 + R1 * k2;
+                    const int u = (k < N / 2) ? k : k - N;                   // signed bin
+                    const int p = u + half;                                  // centre order
+                    if (p < 0 || p >= P.K) continue;                         // keep the central K channels (L611)
+                    float2 v = y[bitrev(k2, ilog2(R2))];
+                    if (SCALE) {
+                        const float f = __ldg(&P.sw[p]);                     // sqrt(w_p): shared edge / DC exclusion
+                        v.x *= f;
+                        v.y *= f;
+                    }
+                    ybase[((size_t)p * P.T + t) * P.pitch2] = __floats2half2_rn(v.x, v.y);
+                }
+            }
+        }
+        __syncthreads();                                              // ex consumed; raw(t+1) visible
     }
 }
 

@@ -98,10 +98,33 @@ int upload(T **dptr, const std::vector<T> &h)
     return MWAX_OK;
 }
 
-using F64 = mwax::FPow2Config<64, 8, 16>;
-using F128 = mwax::FPow2Config<128, 8, 16>;
-using F256 = mwax::FPow2Config<256, 16, 32>;
-using F512 = mwax::FPow2Config<512, 16, 32>;
+// power-of-two register kernel: (N, R1, PTS) per supported length; FULL = every bin kept, SCALE = sw[] applied
+template <int N, int R1, int PTS>
+int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, int groups, int chunks, cudaStream_t st)
+{
+    using C = mwax::FPow2Config<N, R1, PTS>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<N, R1, PTS, true, false>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<N, R1, PTS, true, true>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<N, R1, PTS, false, true>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e != cudaSuccess) return MWAX_ERR_CUDA;
+        attr_set = true;
+    }
+    dim3 grid(groups, chunks);
+    if (full && !scale)
+        mwax::f_stage_pow2_kernel<N, R1, PTS, true, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+    else if (full)
+        mwax::f_stage_pow2_kernel<N, R1, PTS, true, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+    else
+        mwax::f_stage_pow2_kernel<N, R1, PTS, false, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+    return MWAX_OK;
+}
 
 template <bool kInt8, int BN>
 int launch_x(const CUtensorMap &tmap, const mwax::XParams &xp, int sm_count, cudaStream_t st)
@@ -280,18 +303,8 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     h->f_kind = 0;
     if (const char *e = getenv("MWAX_F_GENERIC")) { if (atoi(e) == 1) n_fft = -n_fft; }
     cudaError_t ae = cudaSuccess;
-    switch (n_fft) {
-        case 64: h->f_kind = 64; h->f_smem = F64::SMEM_BYTES;
-            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<64, 8, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, F64::SMEM_BYTES); break;
-        case 128: h->f_kind = 128; h->f_smem = F128::SMEM_BYTES;
-            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<128, 8, 16>, cudaFuncAttributeMaxDynamicSharedMemorySize, F128::SMEM_BYTES); break;
-        case 256: h->f_kind = 256; h->f_smem = F256::SMEM_BYTES;
-            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<256, 16, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, F256::SMEM_BYTES); break;
-        case 512: h->f_kind = 512; h->f_smem = F512::SMEM_BYTES;
-            ae = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<512, 16, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, F512::SMEM_BYTES); break;
-        default:
-            ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
-    }
+    if (n_fft == 64 || n_fft == 128 || n_fft == 256 || n_fft == 512) h->f_kind = n_fft;
+    else ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
     if (n_fft < 0) n_fft = -n_fft;
     if (ae != cudaSuccess) { g_last_error = MWAX_ERR_CUDA; delete h; return nullptr; }
     // twiddles exp(-2 pi i m / N), computed in double
@@ -333,7 +346,7 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
     if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
     mwax::FParams fp;
     fp.volt = d_volt; fp.row_pitch = (long long)row_pitch; fp.sample0 = 0;
-    fp.n_inputs = h->n; fp.N = h->N; fp.K = h->K; fp.T = h->T; fp.G = h->G;
+    fp.n_inputs = h->n; fp.N = h->N; fp.K = h->K; fp.T = h->T; fp.G = h->G; fp.frames_per_cta = 1;
     fp.n_pass = (int)h->radix.size();
     for (int i = 0; i < fp.n_pass; ++i) fp.radix[i] = h->radix[i];
     fp.vec_ok = (h->N % 8 == 0) && (row_pitch % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_volt) & 15u) == 0);
@@ -341,13 +354,22 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
     fp.Y = reinterpret_cast<__half2 *>(h->d_Y); fp.pitch2 = h->pitch / 2;
     cudaStream_t st = (cudaStream_t)stream;
     if (h->f_kind) {
-        dim3 grid((h->n + 31) / 32, h->T);
+        // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
+        const int groups = (h->n + 31) / 32;
+        long long fpc = ((long long)groups * h->T) / ((long long)h->sm_count * 24);
+        if (fpc < 1) fpc = 1;
+        if (fpc > 32) fpc = 32;
+        fp.frames_per_cta = (int)fpc;
+        const int chunks = (h->T + (int)fpc - 1) / (int)fpc;
+        const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
+        int rc;
         switch (h->f_kind) {
-            case 64: mwax::f_stage_pow2_kernel<64, 8, 16><<<grid, F64::THREADS, F64::SMEM_BYTES, st>>>(fp); break;
-            case 128: mwax::f_stage_pow2_kernel<128, 8, 16><<<grid, F128::THREADS, F128::SMEM_BYTES, st>>>(fp); break;
-            case 256: mwax::f_stage_pow2_kernel<256, 16, 32><<<grid, F256::THREADS, F256::SMEM_BYTES, st>>>(fp); break;
-            default: mwax::f_stage_pow2_kernel<512, 16, 32><<<grid, F512::THREADS, F512::SMEM_BYTES, st>>>(fp); break;
+            case 64: rc = launch_f_pow2<64, 8, 16>(fp, full, scale, groups, chunks, st); break;
+            case 128: rc = launch_f_pow2<128, 8, 16>(fp, full, scale, groups, chunks, st); break;
+            case 256: rc = launch_f_pow2<256, 16, 32>(fp, full, scale, groups, chunks, st); break;
+            default: rc = launch_f_pow2<512, 16, 32>(fp, full, scale, groups, chunks, st); break;
         }
+        if (rc != MWAX_OK) return rc;
     } else {
         dim3 grid((h->n + h->G - 1) / h->G, h->T);
         mwax::f_stage_generic_kernel<<<grid, 256, h->f_smem, st>>>(fp);
