@@ -15,6 +15,7 @@
 #include "../../include/mwax_corr.h"
 #include "f_stage.cuh"
 #include "f_stage_pow2.cuh"
+#include "f_stage_6400.cuh"
 #include "x_stage.cuh"
 
 namespace {
@@ -126,6 +127,34 @@ int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, int groups, in
     return MWAX_OK;
 }
 
+template <int TPT>
+int launch_f_6400(const mwax::FParams &fp, bool full, bool scale, int sm_count, cudaStream_t st)
+{
+    using C = mwax::F6400;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(mwax::f_stage_6400_kernel<true, false, TPT>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mwax::f_stage_6400_kernel<true, true, TPT>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e == cudaSuccess)
+            e = cudaFuncSetAttribute(mwax::f_stage_6400_kernel<false, true, TPT>,
+                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e != cudaSuccess) return MWAX_ERR_CUDA;
+        attr_set = true;
+    }
+    // persistent CTAs, one per SM; item = (frame t, group of 4 inputs), groups fastest, so that the eight groups
+    // sharing a 128-byte line of Y run in the same wave
+    const long long items = (long long)((fp.n_inputs + C::G - 1) / C::G) * fp.T;
+    const int grid = (int)(items < sm_count ? items : sm_count);
+    const int thr = C::THREADS / TPT;
+    if (full && !scale) mwax::f_stage_6400_kernel<true, false, TPT><<<grid, thr, C::SMEM_BYTES, st>>>(fp);
+    else if (full) mwax::f_stage_6400_kernel<true, true, TPT><<<grid, thr, C::SMEM_BYTES, st>>>(fp);
+    else mwax::f_stage_6400_kernel<false, true, TPT><<<grid, thr, C::SMEM_BYTES, st>>>(fp);
+    return MWAX_OK;
+}
+
 template <bool kInt8, int BN>
 int launch_x(const CUtensorMap &tmap, const mwax::XParams &xp, int sm_count, cudaStream_t st)
 {
@@ -156,6 +185,7 @@ struct mwax_corr {
     int last_cuda;
     bool tables_ready;
     // F plan
+    int f_tpt;         // N = 6400 kernel: 80-point transforms per thread and pass
     int f_kind;        // 0 = generic Stockham kernel, else the power-of-two register kernel for that N
     float in_scale;
     int chan_scale;
@@ -164,6 +194,7 @@ struct mwax_corr {
     std::vector<int> radix;
     // device tables
     float2 *d_tw;
+    float2 *d_tw2;
     float *d_sw;
     int *d_tap_start;
     float *d_scale;
@@ -301,9 +332,11 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     h->G = G;
     h->f_smem = (size_t)2 * G * n_fft * sizeof(float2);
     h->f_kind = 0;
+    h->f_tpt = 2;
+    if (const char *e = getenv("MWAX_F6400_TPT")) { if (atoi(e) == 1) h->f_tpt = 1; }
     if (const char *e = getenv("MWAX_F_GENERIC")) { if (atoi(e) == 1) n_fft = -n_fft; }
     cudaError_t ae = cudaSuccess;
-    if (n_fft == 64 || n_fft == 128 || n_fft == 256 || n_fft == 512) h->f_kind = n_fft;
+    if (n_fft == 64 || n_fft == 128 || n_fft == 256 || n_fft == 512 || n_fft == 6400) h->f_kind = n_fft;
     else ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
     if (n_fft < 0) n_fft = -n_fft;
     if (ae != cudaSuccess) { g_last_error = MWAX_ERR_CUDA; delete h; return nullptr; }
@@ -314,6 +347,18 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
         tw[m] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
     }
     if ((g_last_error = upload(&h->d_tw, tw)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
+    if (h->f_kind == 6400) {
+        // inter-pass twiddles of the 80 x 80 kernel, [k1][n2], with the F-stage scale s folded in
+        const int lg = (int)std::ceil(std::log2((double)n_fft) / 2.0);
+        const double s = std::ldexp(1.0, -lg);
+        std::vector<float2> tw2(6400);
+        for (int k1 = 0; k1 < 80; ++k1)
+            for (int n2 = 0; n2 < 80; ++n2) {
+                const double a = 2.0 * M_PI * (double)(k1 * n2) / 6400.0;
+                tw2[k1 * 80 + n2] = make_float2((float)(s * std::cos(a)), (float)(-s * std::sin(a)));
+            }
+        if ((g_last_error = upload(&h->d_tw2, tw2)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
+    }
     // workspace Y[K][T][pitch] fp16, zeroed once (pad columns stay zero)
     h->y_bytes = (size_t)n_keep * t_int * h->pitch * sizeof(__half);
     if (cudaMalloc(reinterpret_cast<void **>(&h->d_Y), h->y_bytes) != cudaSuccess) {
@@ -350,10 +395,15 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
     fp.n_pass = (int)h->radix.size();
     for (int i = 0; i < fp.n_pass; ++i) fp.radix[i] = h->radix[i];
     fp.vec_ok = (h->N % 8 == 0) && (row_pitch % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_volt) & 15u) == 0);
-    fp.tw = h->d_tw; fp.sw = h->d_sw; fp.in_scale = h->in_scale; fp.chan_scale = h->chan_scale;
+    fp.tw = h->d_tw; fp.tw2 = h->d_tw2; fp.sw = h->d_sw; fp.in_scale = h->in_scale; fp.chan_scale = h->chan_scale;
     fp.Y = reinterpret_cast<__half2 *>(h->d_Y); fp.pitch2 = h->pitch / 2;
     cudaStream_t st = (cudaStream_t)stream;
-    if (h->f_kind) {
+    if (h->f_kind == 6400) {
+        const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
+        int rc = h->f_tpt == 2 ? launch_f_6400<2>(fp, full, scale, h->sm_count, st)
+                               : launch_f_6400<1>(fp, full, scale, h->sm_count, st);
+        if (rc != MWAX_OK) return rc;
+    } else if (h->f_kind) {
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
         const int groups = (h->n + 31) / 32;
         long long fpc = ((long long)groups * h->T) / ((long long)h->sm_count * 24);
@@ -461,6 +511,7 @@ int mwax_corr_destroy(mwax_corr_t *h)
     if (!h) return MWAX_OK;
     free_tables(h);
     cudaFree(h->d_tw);
+    cudaFree(h->d_tw2);
     cudaFree(h->d_Y);
     cudaFree(h->d_in);
     cudaFree(h->d_out);
