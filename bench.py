@@ -43,7 +43,7 @@ def load_peaks():
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
 
-    def __init__(self, index: int, period: float = 0.05):
+    def __init__(self, index: int, period: float = 0.01):
         super().__init__(daemon=True)
         self.index, self.period = index, period
         self.samples, self.reasons, self.max_mhz = [], set(), None
@@ -97,93 +97,113 @@ def physical_gpu_index(local_rank: int) -> int:
     return local_rank
 
 
+def _oracle_sample(cfg, budget_s):
+    """Pick a bounded sample of the workload (all inputs; the first t_s spectra of dump 0; if one spectrum is
+    still too slow, the central K_s fine channels only) that the oracle finishes in about budget_s seconds."""
+    from oracle import oracle
+    from paper_2303_11557_b200 import synth
+    N, K, F = cfg.n_fft, cfg.n_keep, cfg.f_avg
+    spec = cfg.spec()
+    n_cal = 8 if K <= 1024 else 1
+    spec.n_samples = n_cal * N
+    volt1 = synth.gauss_voltages(spec)
+    k_cal = K if K <= 1024 else max(F, (1024 // F) * F)    # calibration: one spectrum, at most 1024 channels
+    oracle.fx(volt1, N, k_cal, 1, F)                          # warm the library and the thread pool
+    t0 = time.perf_counter()
+    oracle.fx(volt1, N, k_cal, 1, F)
+    c1 = time.perf_counter() - t0
+    fixed, per_spec = 0.0, 1.25 * c1 * K / k_cal             # X stage dominates: linear in channels and spectra
+    if n_cal > 1:                                            # cost = fixed (output allocation, averaging) + slope * spectra
+        t0 = time.perf_counter()
+        oracle.fx(volt1, N, k_cal, n_cal, F)
+        c2 = time.perf_counter() - t0
+        per_spec = max(1e-4, 1.25 * (c2 - c1) / (n_cal - 1))
+        fixed = max(0.0, c1 - per_spec)
+    t_s, k_s = max(1, int((budget_s - fixed) / per_spec)), K
+    if per_spec > budget_s:
+        k_s = max(F, int(K * budget_s / per_spec) // F * F)
+    t_s = min(t_s, cfg.t_int)
+    spec.n_samples = t_s * N
+    return synth.gauss_voltages(spec), t_s, k_s
+
+
+def _oracle_rate(cfg, volt, t_s, k_s):
+    from oracle import oracle
+    N, K, F = cfg.n_fft, cfg.n_keep, cfg.f_avg
+    t0 = time.perf_counter()
+    oracle.fx(volt, N, k_s, t_s, F)
+    sec = time.perf_counter() - t0
+    data_seconds = t_s * N / SAMPLE_RATE * (k_s / K)         # fraction of one coarse channel-second processed
+    sample = (f"all {cfg.n_inputs} inputs, central {k_s} of {K} fine channels, first {t_s} spectra "
+              f"({t_s * N / SAMPLE_RATE * 1e3:.2f} ms of data) of dump 0")
+    return data_seconds / sec, sec, sample
+
+
 def run_reference(args):
     """The oracle, as it stands, on the host cores: a bounded sample of the workload per step."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import numpy as np
     from oracle import oracle
     from paper_2303_11557_b200 import synth
     cfg = synth.CONFIGS[args.workload]
-    N, K, F = cfg.n_fft, cfg.n_keep, cfg.f_avg
-    # sample: all inputs, all channels, the first t_s spectra of dump 0 (t_s chosen for ~5-10 s per step)
-    t_s = 24 if args.workload == "C3" else 1
-    spec = cfg.spec()
-    spec.n_samples = t_s * N
-    volt = synth.gauss_voltages(spec)
     oracle.build()
-    times = []
+    budget = min(10.0, 120.0 / (args.warmup + args.steps))  # whole run ~2 minutes
+    volt, t_s, k_s = _oracle_sample(cfg, budget)
+    vals, secs = [], []
+    sample = ""
     for it in range(args.warmup + args.steps):
-        t0 = time.perf_counter()
-        oracle.fx(volt, N, K, t_s, F)
-        t1 = time.perf_counter()
+        v, sec, sample = _oracle_rate(cfg, volt, t_s, k_s)
         if it >= args.warmup:
-            times.append(t1 - t0)
-    sec = sum(times) / len(times)
-    data_seconds = t_s * N / SAMPLE_RATE
-    value = data_seconds / sec
-    sample = f"all {cfg.n_inputs} inputs, all {K} fine channels, first {t_s} spectra ({data_seconds*1e3:.2f} ms of data) of dump 0"
+            vals.append(v)
+            secs.append(sec)
+    sec = sum(secs) / len(secs)
+    value = sum(vals) / len(vals)
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_fft": N, "n_keep": K, "f_avg": F,
-                       "sample": sample},
+            "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_fft": cfg.n_fft, "n_keep": cfg.n_keep,
+                       "f_avg": cfg.f_avg, "sample": sample},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
 
-def cpu_baseline(cfg, budget_spectra):
-    import numpy as np
+def cpu_baseline(cfg, budget_s=15.0):
     from oracle import oracle
-    from paper_2303_11557_b200 import synth
     oracle.build()
-    N, K, F = cfg.n_fft, cfg.n_keep, cfg.f_avg
-    spec = cfg.spec()
-    spec.n_samples = budget_spectra * N
-    volt = synth.gauss_voltages(spec)
-    t0 = time.perf_counter()
-    oracle.fx(volt, N, K, budget_spectra, F)
-    sec = time.perf_counter() - t0
-    data_seconds = budget_spectra * N / SAMPLE_RATE
-    return {"value": data_seconds / sec, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
-            "sample": f"all {cfg.n_inputs} inputs, all {K} fine channels, first {budget_spectra} spectra "
-                      f"({data_seconds*1e3:.2f} ms of data) in {sec:.1f} s",
-            "seconds": sec}
+    volt, t_s, k_s = _oracle_sample(cfg, budget_s)
+    value, sec, sample = _oracle_rate(cfg, volt, t_s, k_s)
+    return {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": sample + f" in {sec:.1f} s", "seconds": sec}
 
 
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C3", "C4"])
-    ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-e2e", action="store_true")
-    args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 0)
+def load_traffic():
+    """Per-launch DRAM bytes (dram__bytes_read.sum + dram__bytes_write.sum) of each kernel from the committed
+    `ncu --set full` captures: profiles/traffic.csv, columns workload,stage,kernel,dram_bytes_per_launch."""
+    out = {}
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    if os.path.exists(path):
+        with open(path) as f:
+            for ln in f:
+                if ln.startswith("#") or not ln.strip():
+                    continue
+                w, stage, _k, b = [x.strip() for x in ln.split(",")][:4]
+                try:
+                    out[(w, stage)] = float(b)
+                except ValueError:
+                    pass
+    return out
 
-    if args.impl == "reference":
-        run_reference(args)
-        return
 
-    import numpy as np
+def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
+    """Time `steps` passes of the whole hot path over workload `wl` (device-resident input), per-stage CUDA events
+    inside the timed region, then the end-to-end leg through mwax_corr_process_host."""
     import torch
     import torch.distributed as dist
     from paper_2303_11557_b200 import corr, synth
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-
-    cfg = synth.CONFIGS[args.workload]
+    cfg = synth.CONFIGS[wl]
     n, N, K, T, F, D = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg, cfg.n_dumps
     B = n * (n + 1) // 2
     C = K // F
@@ -197,27 +217,27 @@ def main():
     h = corr.MwaxCorr(n, N, K, T, F)
     vis = h.new_output(n_dumps=D)
     stream = torch.cuda.current_stream()
+    sp = int(stream.cuda_stream)
     dump_bytes = T * N * 2
+    L = corr.lib()
 
     def step(events=None):
         for d in range(D):
-            v = volt[0, :, d * T * N:, :]
-            ptr_off = d * dump_bytes
             if events is not None:
                 e0, e1, e2 = events[d]
                 e0.record(stream)
-            corr._check(corr.lib().mwax_corr_f_stage(h._h, volt.data_ptr() + ptr_off, row, int(stream.cuda_stream)), "f_stage", h._h)
+            corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr() + d * dump_bytes, row, sp), "f_stage", h._h)
             if events is not None:
                 e1.record(stream)
-            corr._check(corr.lib().mwax_corr_x_stage(h._h, vis[0, d].data_ptr(), int(stream.cuda_stream)), "x_stage", h._h)
+            corr._check(L.mwax_corr_x_stage(h._h, vis[0, d].data_ptr(), sp), "x_stage", h._h)
             if events is not None:
                 e2.record(stream)
 
-    for _ in range(args.warmup):
+    for _ in range(warmup):
         step()
     torch.cuda.synchronize()
 
-    evs = [[tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(D)] for _ in range(args.steps)]
+    evs = [[tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(D)] for _ in range(steps)]
     sampler = ClockSampler(physical_gpu_index(local_rank))
     if world > 1:
         dist.barrier()
@@ -226,7 +246,7 @@ def main():
     t_start = torch.cuda.Event(enable_timing=True)
     t_end = torch.cuda.Event(enable_timing=True)
     t_start.record(stream)
-    for k in range(args.steps):
+    for k in range(steps):
         step(evs[k])
     t_end.record(stream)
     torch.cuda.synchronize()
@@ -238,17 +258,20 @@ def main():
         tt = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
         total_ms = float(tt.item())
-    ms_per_step = total_ms / args.steps
-    f_ms = [e[0].elapsed_time(e[1]) for s in evs for e in s]
-    x_ms = [e[1].elapsed_time(e[2]) for s in evs for e in s]
+    ms_per_step = total_ms / steps
+    f_ms = [e[0].elapsed_time(e[1]) for s_ in evs for e in s_]
+    x_ms = [e[1].elapsed_time(e[2]) for s_ in evs for e in s_]
     f_avg_ms, x_avg_ms = sum(f_ms) / len(f_ms), sum(x_ms) / len(x_ms)
-    value = world * data_seconds / (ms_per_step * 1e-3)
+    res = {"cfg": cfg, "value": world * data_seconds / (ms_per_step * 1e-3), "ms_per_step": ms_per_step,
+           "total_ms": total_ms, "f_ms": f_avg_ms, "x_ms": x_avg_ms, "clocks": clocks,
+           "launches": steps * D * h.launches_per_process(), "in_bytes": host.numel(),
+           "ws_bytes": h.workspace_bytes(), "e2e": None,
+           "input_samples_per_s": world * n * row / (ms_per_step * 1e-3)}
 
     # ---- e2e through the public host-buffer call (H2D + D2H inside the timed region)
-    e2e = None
-    if not args.no_e2e:
+    if do_e2e:
         hvis = torch.empty((1, D, C, B, 2), dtype=torch.float32).pin_memory()
-        e_steps = max(2, min(args.steps, 5))
+        e_steps = max(2, min(steps, 5))
         h.process_host(host, hvis, D, 1)          # warm-up (allocates staging)
         torch.cuda.synchronize()
         if world > 1:
@@ -265,48 +288,106 @@ def main():
             tt = torch.tensor([e_ms], device="cuda", dtype=torch.float64)
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             e_ms = float(tt.item())
-        e2e = {"value": world * data_seconds / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.numel(),
-               "d2h_bytes_per_step": hvis.numel() * 4, "ms_per_step": e_ms, "steps": e_steps}
+        res["e2e"] = {"value": world * data_seconds / (e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.numel(),
+                      "d2h_bytes_per_step": hvis.numel() * 4, "ms_per_step": e_ms, "steps": e_steps}
+        del hvis
+    h.destroy()
+    del volt, vis, host
+    torch.cuda.empty_cache()
+    return res
+
+
+def rooflines(res, peaks, traffic, wl):
+    """F stage = 6 bytes per kept input sample against HBM; X stage = 8 n(n+1)/2 flops per
+    (fine channel, time) sample against the dense 16-bit tensor peak."""
+    cfg = res["cfg"]
+    n, N, K, T = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int
+    B = n * (n + 1) // 2
+    peak_kind = "sustained" if res["total_ms"] >= 1000.0 else "burst"
+    tensor_peak = peaks["tensor_sustained"] if peak_kind == "sustained" else peaks["tensor_burst"]
+    x_ach = 8.0 * B * K * T / (res["x_ms"] * 1e-3) / 1e12
+    f_ach = (n * T * N * 2.0 + n * T * K * 4.0) / (res["f_ms"] * 1e-3) / 1e9
+    f_name = {6400: "f_stage_6400p3_kernel"}.get(N, "f_stage_pow2_kernel" if N in (64, 128, 256, 512) else "f_stage_generic_kernel")
+    roof_x = {"kernel": "x_stage_kernel<fp16,256>", "bound": "tensor", "achieved": x_ach, "peak": tensor_peak,
+              "unit": "TFLOP/s", "frac": x_ach / tensor_peak, "traffic": traffic.get((wl, "x")),
+              "avg_launch_ms": res["x_ms"], "peak_source": f"{peaks['source']} bf16 {peak_kind} (MEASURED_PEAKS.json)",
+              "frac_of_nominal_2250": x_ach / 2250.0,
+              "executed_over_algorithmic": "tiles cover 1.25x the lower triangle at n=512 (DESIGN.md 5.2)"}
+    roof_f = {"kernel": f_name, "bound": "hbm", "achieved": f_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+              "frac": f_ach / peaks["hbm_gbs"], "traffic": traffic.get((wl, "f")), "avg_launch_ms": res["f_ms"],
+              "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)"}
+    return roof_f, roof_x
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C3", choices=["C3", "C4"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the second workload reported under 'workloads'")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 0)
+
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    res = measure(args.workload, args.steps, args.warmup, world, rank, local_rank, not args.no_e2e)
+    other = None
+    if not args.no_extra:
+        wl2 = "C4" if args.workload == "C3" else "C3"
+        other = (wl2, measure(wl2, max(3, args.steps // 4), args.warmup, world, rank, local_rank, False))
 
     if rank == 0:
         peaks = load_peaks()
-        timed_s = total_ms * 1e-3
-        peak_kind = "sustained" if timed_s >= 1.0 else "burst"
-        tensor_peak = peaks["tensor_sustained"] if peak_kind == "sustained" else peaks["tensor_burst"]
-        # dominant kernel: X stage.  Algorithmic flops: 8 * n(n+1)/2 per (fine channel, time) sample
-        x_flops = 8.0 * B * K * T
-        x_ach = x_flops / (x_avg_ms * 1e-3) / 1e12
-        f_bytes = n * T * N * 2.0 + n * T * K * 4.0          # 2 B in + 4 B out per kept sample
-        f_ach = f_bytes / (f_avg_ms * 1e-3) / 1e9
-        x_dom = x_avg_ms >= f_avg_ms
-        roof_x = {"kernel": "x_stage_kernel<fp16>", "bound": "tensor", "achieved": x_ach, "peak": tensor_peak,
-                  "unit": "TFLOP/s", "frac": x_ach / tensor_peak, "traffic": None, "avg_launch_ms": x_avg_ms,
-                  "peak_source": f"{peaks['source']} bf16 {peak_kind} (MEASURED_PEAKS.json)",
-                  "frac_of_nominal_2250": x_ach / 2250.0}
-        roof_f = {"kernel": "f_stage_kernel", "bound": "hbm", "achieved": f_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
-                  "frac": f_ach / peaks["hbm_gbs"], "traffic": None, "avg_launch_ms": f_avg_ms,
-                  "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)"}
-        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-                "dtype": "f16 operands, f32 accumulate (FFT in f32)", "data": "synthetic",
-                "config": {"workload": cfg.name, "n_inputs": n, "n_fft": N, "n_keep": K, "t_int": T, "f_avg": F,
-                           "dumps_per_step": D, "seconds_of_data_per_step": data_seconds,
-                           "coarse_channels_per_gpu_per_step": 1, "parallelism": f"coarse-channel x{world}",
+        traffic = load_traffic()
+        cfg = res["cfg"]
+        roof_f, roof_x = rooflines(res, peaks, traffic, args.workload)
+        x_dom = res["x_ms"] >= res["f_ms"]
+        line = {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f16 operands, f32 accumulate (FFT in f32)", "data": "synthetic",
+                "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_fft": cfg.n_fft, "n_keep": cfg.n_keep,
+                           "t_int": cfg.t_int, "f_avg": cfg.f_avg, "dumps_per_step": cfg.n_dumps,
+                           "seconds_of_data_per_step": cfg.seconds_of_data, "coarse_channels_per_gpu_per_step": 1,
+                           "parallelism": f"coarse-channel x{world}",
                            "l2": "inputs larger than L2 (%.2f GB in, %.2f GB workspace per dump)" %
-                                 (host.numel() / 1e9, h.workspace_bytes() / 1e9)},
-                "input_samples_per_s": world * n * row / (ms_per_step * 1e-3),
-                "gpu_launches": args.steps * D * h.launches_per_process(),
-                "clocks": clocks,
+                                 (res["in_bytes"] / 1e9, res["ws_bytes"] / 1e9)},
+                "input_samples_per_s": res["input_samples_per_s"],
+                "gpu_launches": res["launches"],
+                "clocks": res["clocks"],
                 "roofline": roof_x if x_dom else roof_f,
                 "stages": {"f": roof_f, "x": roof_x},
                 "paper_context": "MWAX on 1 x A40 + 2 x Epyc 7F72: 5.9 s per 8 s subfile at 256 tiles, 1 s/10 kHz mode "
                                  "=> 1 coarse channel per GPU in real time (PAPER.md Table 2 L531-545)"}
-        if e2e is not None:
-            line["e2e"] = e2e
+        if other is not None:
+            wl2, r2 = other
+            rf2, rx2 = rooflines(r2, peaks, traffic, wl2)
+            line["workloads"] = {r2["cfg"].name: {"value": r2["value"], "ms_per_step": r2["ms_per_step"],
+                                                   "seconds_of_data_per_step": r2["cfg"].seconds_of_data,
+                                                   "steps": max(3, args.steps // 4), "clocks": r2["clocks"],
+                                                   "stages": {"f": rf2, "x": rx2}}}
+        if res["e2e"] is not None:
+            line["e2e"] = res["e2e"]
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline(cfg, 24 if args.workload == "C3" else 1)
+            line["cpu_baseline"] = cpu_baseline(cfg)
         print(json.dumps(line), flush=True)
-    h.destroy()
     if world > 1:
         dist.destroy_process_group()
 

@@ -25,12 +25,13 @@ struct FParams {
     int radix[16];
     int vec_ok;              // 16-byte loads allowed
     const float2 *tw;        // [N] exp(-2 pi i m / N)
-    const float2 *tw2;       // N = 6400 kernel: [k1][n2] s * exp(-2 pi i n2 k1 / 6400), 80 x 80
+    const unsigned *swcode;  // N = 6400 three-pass kernel, K == N: [c = k mod 400] 2 bits per k3 = k / 400: 0 -> 1, 1 -> sqrt(1/2), 2 -> 0
     const float *sw;         // [K] per-position factor sqrt(w_p): 1, sqrt(1/2) on a shared edge, 0 for excluded DC
     float in_scale;          // s: power-of-two F-stage scale (keeps fp16 in range)
     int chan_scale;          // 0 when every sw[p] == 1
     __half2 *Y;              // [K][T][pitch2]
     int pitch2;              // half2 (complex) elements per Y row
+    unsigned y_p_stride, y_t_stride;   // half2 elements between channel positions / between spectra (p3 kernel)
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)

@@ -15,7 +15,7 @@
 #include "../../include/mwax_corr.h"
 #include "f_stage.cuh"
 #include "f_stage_pow2.cuh"
-#include "f_stage_6400.cuh"
+#include "f_stage_6400p3.cuh"
 #include "x_stage.cuh"
 
 namespace {
@@ -127,32 +127,39 @@ int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, int groups, in
     return MWAX_OK;
 }
 
-template <int TPT>
-int launch_f_6400(const mwax::FParams &fp, bool full, bool scale, int sm_count, cudaStream_t st)
+template <bool FULL, bool SCALE, int Q>
+int launch_f_6400p3_q(const mwax::FParams &fp, cudaStream_t st)
 {
-    using C = mwax::F6400;
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(mwax::f_stage_6400_kernel<true, false, TPT>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mwax::f_stage_6400_kernel<true, true, TPT>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mwax::f_stage_6400_kernel<false, true, TPT>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e != cudaSuccess) return MWAX_ERR_CUDA;
-        attr_set = true;
+    using C = mwax::F6400P3;
+    auto kern = mwax::f_stage_6400p3_kernel<FULL, SCALE, Q>;
+    static int max_clusters = 0;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = Q; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (!max_clusters) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+            return MWAX_ERR_CUDA;
+        cfg.gridDim = dim3(Q);
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) return MWAX_ERR_CUDA;
+        max_clusters = n;
     }
-    // persistent CTAs, one per SM; item = (frame t, group of 4 inputs), groups fastest, so that the eight groups
-    // sharing a 128-byte line of Y run in the same wave
-    const long long items = (long long)((fp.n_inputs + C::G - 1) / C::G) * fp.T;
-    const int grid = (int)(items < sm_count ? items : sm_count);
-    const int thr = C::THREADS / TPT;
-    if (full && !scale) mwax::f_stage_6400_kernel<true, false, TPT><<<grid, thr, C::SMEM_BYTES, st>>>(fp);
-    else if (full) mwax::f_stage_6400_kernel<true, true, TPT><<<grid, thr, C::SMEM_BYTES, st>>>(fp);
-    else mwax::f_stage_6400_kernel<false, true, TPT><<<grid, thr, C::SMEM_BYTES, st>>>(fp);
-    return MWAX_OK;
+    // persistent clusters; item = (frame t, group of 4 Q inputs), groups fastest
+    const long long items = (long long)((fp.n_inputs + C::G * Q - 1) / (C::G * Q)) * fp.T;
+    const int n_cl = (int)(items < max_clusters ? items : max_clusters);
+    cfg.gridDim = dim3(n_cl * Q);
+    return cudaLaunchKernelEx(&cfg, kern, fp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
+}
+
+template <int Q>
+int launch_f_6400p3(const mwax::FParams &fp, bool full, bool scale, cudaStream_t st)
+{
+    if (full && !scale) return launch_f_6400p3_q<true, false, Q>(fp, st);
+    if (full) return launch_f_6400p3_q<true, true, Q>(fp, st);
+    return launch_f_6400p3_q<false, true, Q>(fp, st);
 }
 
 template <bool kInt8, int BN>
@@ -185,7 +192,6 @@ struct mwax_corr {
     int last_cuda;
     bool tables_ready;
     // F plan
-    int f_tpt;         // N = 6400 kernel: 80-point transforms per thread and pass
     int f_kind;        // 0 = generic Stockham kernel, else the power-of-two register kernel for that N
     float in_scale;
     int chan_scale;
@@ -194,7 +200,8 @@ struct mwax_corr {
     std::vector<int> radix;
     // device tables
     float2 *d_tw;
-    float2 *d_tw2;
+    unsigned *d_swcode;
+    int f_p3;          // N = 6400: cluster size Q (2, 4, 8) of the three-pass 20 x 20 x 16 kernel
     float *d_sw;
     int *d_tap_start;
     float *d_scale;
@@ -232,6 +239,7 @@ static int note_cuda(int *slot)
 static void free_tables(mwax_corr *h)
 {
     cudaFree(h->d_sw); h->d_sw = nullptr;
+    cudaFree(h->d_swcode); h->d_swcode = nullptr;
     cudaFree(h->d_tap_start); h->d_tap_start = nullptr;
     cudaFree(h->d_scale); h->d_scale = nullptr;
     cudaFree(h->d_tiles); h->d_tiles = nullptr;
@@ -277,6 +285,16 @@ static int build_tables(mwax_corr *h)
     h->n_tiles = (int)tiles.size() / 2;
     int rc;
     if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
+    if (h->N == 6400 && K == 6400) {
+        // the three-pass kernel takes sqrt(w_p) as 2-bit codes, one word per c = k mod 400, field k3 = k / 400
+        std::vector<unsigned> code(400, 0u);
+        for (int k = 0; k < 6400; ++k) {
+            const float v = sw[k < 3200 ? k + 3200 : k - 3200];
+            const unsigned cd = v == 1.0f ? 0u : (v == 0.0f ? 2u : 1u);
+            code[k % 400] |= cd << (2 * (k / 400));
+        }
+        if ((rc = upload(&h->d_swcode, code)) != MWAX_OK) return rc;
+    }
     if ((rc = upload(&h->d_tap_start, tap)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_scale, scale)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_tiles, tiles)) != MWAX_OK) return rc;
@@ -332,8 +350,6 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     h->G = G;
     h->f_smem = (size_t)2 * G * n_fft * sizeof(float2);
     h->f_kind = 0;
-    h->f_tpt = 2;
-    if (const char *e = getenv("MWAX_F6400_TPT")) { if (atoi(e) == 1) h->f_tpt = 1; }
     if (const char *e = getenv("MWAX_F_GENERIC")) { if (atoi(e) == 1) n_fft = -n_fft; }
     cudaError_t ae = cudaSuccess;
     if (n_fft == 64 || n_fft == 128 || n_fft == 256 || n_fft == 512 || n_fft == 6400) h->f_kind = n_fft;
@@ -348,16 +364,8 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     }
     if ((g_last_error = upload(&h->d_tw, tw)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
     if (h->f_kind == 6400) {
-        // inter-pass twiddles of the 80 x 80 kernel, [k1][n2], with the F-stage scale s folded in
-        const int lg = (int)std::ceil(std::log2((double)n_fft) / 2.0);
-        const double s = std::ldexp(1.0, -lg);
-        std::vector<float2> tw2(6400);
-        for (int k1 = 0; k1 < 80; ++k1)
-            for (int n2 = 0; n2 < 80; ++n2) {
-                const double a = 2.0 * M_PI * (double)(k1 * n2) / 6400.0;
-                tw2[k1 * 80 + n2] = make_float2((float)(s * std::cos(a)), (float)(-s * std::sin(a)));
-            }
-        if ((g_last_error = upload(&h->d_tw2, tw2)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
+        h->f_p3 = 2;   // cluster size of the three-pass kernel: 2 measured fastest on B200
+        if (const char *e = getenv("MWAX_F6400_Q")) { const int q = atoi(e); if (q == 2 || q == 4 || q == 8) h->f_p3 = q; }
     }
     // workspace Y[K][T][pitch] fp16, zeroed once (pad columns stay zero)
     h->y_bytes = (size_t)n_keep * t_int * h->pitch * sizeof(__half);
@@ -395,13 +403,14 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
     fp.n_pass = (int)h->radix.size();
     for (int i = 0; i < fp.n_pass; ++i) fp.radix[i] = h->radix[i];
     fp.vec_ok = (h->N % 8 == 0) && (row_pitch % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_volt) & 15u) == 0);
-    fp.tw = h->d_tw; fp.tw2 = h->d_tw2; fp.sw = h->d_sw; fp.in_scale = h->in_scale; fp.chan_scale = h->chan_scale;
+    fp.tw = h->d_tw; fp.swcode = h->d_swcode; fp.sw = h->d_sw; fp.in_scale = h->in_scale; fp.chan_scale = h->chan_scale;
     fp.Y = reinterpret_cast<__half2 *>(h->d_Y); fp.pitch2 = h->pitch / 2;
+    fp.y_p_stride = (unsigned)h->T * (unsigned)(h->pitch / 2); fp.y_t_stride = (unsigned)(h->pitch / 2);
     cudaStream_t st = (cudaStream_t)stream;
     if (h->f_kind == 6400) {
         const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
-        int rc = h->f_tpt == 2 ? launch_f_6400<2>(fp, full, scale, h->sm_count, st)
-                               : launch_f_6400<1>(fp, full, scale, h->sm_count, st);
+        int rc = h->f_p3 == 8 ? launch_f_6400p3<8>(fp, full, scale, st) : h->f_p3 == 4 ? launch_f_6400p3<4>(fp, full, scale, st)
+                                                                        : launch_f_6400p3<2>(fp, full, scale, st);
         if (rc != MWAX_OK) return rc;
     } else if (h->f_kind) {
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
@@ -511,7 +520,6 @@ int mwax_corr_destroy(mwax_corr_t *h)
     if (!h) return MWAX_OK;
     free_tables(h);
     cudaFree(h->d_tw);
-    cudaFree(h->d_tw2);
     cudaFree(h->d_Y);
     cudaFree(h->d_in);
     cudaFree(h->d_out);
