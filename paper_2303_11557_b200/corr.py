@@ -15,7 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libmwax_corr.so")
-_SOURCES = ["mwax_api.cu", "f_stage.cuh", "f_stage_pow2.cuh", "f_stage_6400p3.cuh", "x_stage.cuh", "ptx.cuh"]
+_SOURCES = ["mwax_api.cu", "f_stage.cuh", "f_stage_pow2.cuh", "f_stage_6400p3.cuh", "x_stage.cuh", "x_stage2.cuh", "ptx.cuh"]
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "mwax_corr.h")
 _lib = None
 

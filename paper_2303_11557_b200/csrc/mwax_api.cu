@@ -17,6 +17,7 @@
 #include "f_stage_pow2.cuh"
 #include "f_stage_6400p3.cuh"
 #include "x_stage.cuh"
+#include "x_stage2.cuh"
 
 namespace {
 
@@ -77,17 +78,44 @@ int check_device(int *sm_count)
     return MWAX_OK;
 }
 
-// lower-triangle tile list: G-tile (mi, nj) covers inputs i in [64 mi, 64 mi + 64), j in [bn/2 nj, bn/2 (nj+1))
+// lower-triangle tile list, 4 bytes per tile (mi, nj, w, 0): G rows of inputs [64 mi, 64 mi + 64), G columns of inputs
+// [64 nj, 64 nj + 64 w).  Row block mi needs the columns of inputs [0, 64 (mi + 1)): pairs of 64-input units become
+// 256-wide tiles (w = 2), an odd unit left over on the diagonal a 128-wide one (w = 1), so at n = 512 the tiles cover
+// 1.12x the lower triangle (16 wide + 4 narrow) instead of 1.25x (20 wide).
 void build_tiles(int n, int bn, std::vector<uint8_t> &tiles)
 {
     tiles.clear();
-    const int im = 64, jn = bn / 2;
-    for (int mi = 0; mi * im < n; ++mi)
-        for (int nj = 0; nj * jn < n; ++nj)
-            if (mi * im + im - 1 >= nj * jn) {
-                tiles.push_back((uint8_t)mi);
-                tiles.push_back((uint8_t)nj);
-            }
+    for (int mi = 0; mi * 64 < n; ++mi) {
+        const int units = mi + 1;
+        for (int u = 0; u < units;) {
+            const int w = (bn == 256 && u + 2 <= units) ? 2 : 1;
+            tiles.push_back((uint8_t)mi);
+            tiles.push_back((uint8_t)u);
+            tiles.push_back((uint8_t)w);
+            tiles.push_back(0);
+            u += w;
+        }
+    }
+}
+
+// tile list of the CTA-pair kernel: (mi, nj, 0, 0) in units of 128 inputs, nj <= mi
+void build_pair_tiles(int n, std::vector<uint8_t> &tiles)
+{
+    tiles.clear();
+    for (int mi = 0; mi * 128 < n; ++mi)
+        for (int nj = 0; nj <= mi; ++nj) {
+            tiles.push_back((uint8_t)mi);
+            tiles.push_back((uint8_t)nj);
+            tiles.push_back(0);
+            tiles.push_back(0);
+        }
+}
+
+int want_pair_kernel()
+{
+    // debugging aid: MWAX_X_PAIR=0 selects the single-CTA kernel instead of the cta_group::2 pair kernel
+    const char *e = getenv("MWAX_X_PAIR");
+    return (e && atoi(e) == 0) ? 0 : 1;
 }
 
 template <typename T>
@@ -163,7 +191,7 @@ int launch_f_6400p3(const mwax::FParams &fp, bool full, bool scale, cudaStream_t
 }
 
 template <bool kInt8, int BN>
-int launch_x(const CUtensorMap &tmap, const mwax::XParams &xp, int sm_count, cudaStream_t st)
+int launch_x(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::XParams &xp, int sm_count, cudaStream_t st)
 {
     using C = mwax::XConfig<kInt8, BN>;
     static bool attr_set = false;
@@ -176,8 +204,32 @@ int launch_x(const CUtensorMap &tmap, const mwax::XParams &xp, int sm_count, cud
     const int n_items = xp.n_out * xp.n_tiles;
     if (n_items <= 0) return MWAX_OK;
     const int grid = n_items < sm_count ? n_items : sm_count;
-    mwax::x_stage_kernel<kInt8, BN><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(tmap, xp);
+    mwax::x_stage_kernel<kInt8, BN><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(tmap, tmap_flat, xp);
     return cudaGetLastError() == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
+}
+
+template <bool kInt8>
+int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::XParams &xp, int sm_count, cudaStream_t st)
+{
+    using C = mwax::XPairConfig<kInt8>;
+    auto kern = mwax::x_stage_pair_kernel<kInt8>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+            return MWAX_ERR_CUDA;
+        attr_set = true;
+    }
+    const int n_items = xp.n_out * xp.n_tiles;
+    if (n_items <= 0) return MWAX_OK;
+    int pairs = sm_count / 2;
+    if (n_items < pairs) pairs = n_items;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.gridDim = dim3(2 * pairs); cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, tmap, tmap_flat, xp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
 }
 
 }  // namespace
@@ -206,10 +258,13 @@ struct mwax_corr {
     int *d_tap_start;
     float *d_scale;
     uint8_t *d_tiles;
+    uint8_t *d_ptiles;  // CTA-pair kernel's tile list
+    int n_ptiles, x_pair;
     int n_tiles, n_taps;
     __half *d_Y;
     size_t y_bytes;
-    CUtensorMap tmap;
+    CUtensorMap tmap;       // Y as [p][t][2n]: one channel position per box (rows past T read as zero)
+    CUtensorMap tmap_flat;  // Y as [p T + t][2n]: boxes may run across adjacent channel positions
     // staging for process_host
     int8_t *d_in;
     size_t in_bytes;
@@ -224,7 +279,8 @@ struct mwax_xcorr {
     int last_cuda;
     int *d_tap_start;
     uint8_t *d_tiles;
-    int n_tiles;
+    uint8_t *d_ptiles;
+    int n_tiles, n_ptiles, x_pair;
     int8_t *d_in;
     int32_t *d_out;
 };
@@ -243,6 +299,7 @@ static void free_tables(mwax_corr *h)
     cudaFree(h->d_tap_start); h->d_tap_start = nullptr;
     cudaFree(h->d_scale); h->d_scale = nullptr;
     cudaFree(h->d_tiles); h->d_tiles = nullptr;
+    cudaFree(h->d_ptiles); h->d_ptiles = nullptr;
     h->tables_ready = false;
 }
 
@@ -282,7 +339,7 @@ static int build_tables(mwax_corr *h)
     }
     std::vector<uint8_t> tiles;
     build_tiles(h->n, h->x_bn, tiles);
-    h->n_tiles = (int)tiles.size() / 2;
+    h->n_tiles = (int)tiles.size() / 4;
     int rc;
     if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
     if (h->N == 6400 && K == 6400) {
@@ -298,6 +355,9 @@ static int build_tables(mwax_corr *h)
     if ((rc = upload(&h->d_tap_start, tap)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_scale, scale)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_tiles, tiles)) != MWAX_OK) return rc;
+    build_pair_tiles(h->n, tiles);
+    h->n_ptiles = (int)tiles.size() / 4;
+    if ((rc = upload(&h->d_ptiles, tiles)) != MWAX_OK) return rc;
     h->tables_ready = true;
     return MWAX_OK;
 }
@@ -339,6 +399,7 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     h->avg_mode = MWAX_AVG_CENTRE_SYMMETRIC;
     h->x_bn = 256;
     if (const char *e = getenv("MWAX_X_TILE_N")) { if (atoi(e) == 128) h->x_bn = 128; }
+    h->x_pair = want_pair_kernel();
     h->pitch = ((2 * n_inputs + 63) / 64) * 64;
     h->sm_count = sm;
     h->last_cuda = 0;
@@ -375,6 +436,10 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     cudaMemset(h->d_Y, 0, h->y_bytes);
     if ((g_last_error = encode_z_map(&h->tmap, false, h->d_Y, (uint64_t)h->pitch, (uint64_t)h->pitch * 2,
                                      (uint64_t)t_int, (uint64_t)n_keep, 64)) != MWAX_OK) {
+        mwax_corr_destroy(h); return nullptr;
+    }
+    if ((g_last_error = encode_z_map(&h->tmap_flat, false, h->d_Y, (uint64_t)h->pitch, (uint64_t)h->pitch * 2,
+                                     (uint64_t)t_int * n_keep, 1, 64)) != MWAX_OK) {
         mwax_corr_destroy(h); return nullptr;
     }
     if ((g_last_error = build_tables(h)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
@@ -444,8 +509,14 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
     xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = h->C; xp.n_tiles = h->n_tiles;
     xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = h->n_taps; xp.scale = h->d_scale;
     xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
-    int rc = (h->x_bn == 128) ? launch_x<false, 128>(h->tmap, xp, h->sm_count, (cudaStream_t)stream)
-                              : launch_x<false, 256>(h->tmap, xp, h->sm_count, (cudaStream_t)stream);
+    if (h->x_pair) {
+        xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
+        int rcp = launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
+        if (rcp != MWAX_OK) note_cuda(&h->last_cuda);
+        return rcp;
+    }
+    int rc = (h->x_bn == 128) ? launch_x<false, 128>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream)
+                              : launch_x<false, 256>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
     if (rc != MWAX_OK) note_cuda(&h->last_cuda);
     return rc;
 }
@@ -544,8 +615,13 @@ mwax_xcorr_t *mwax_xcorr_i8_create(int n_inputs, int n_chan, int n_time)
     for (int c = 0; c < n_chan; ++c) tap[c] = c;
     std::vector<uint8_t> tiles;
     build_tiles(n_inputs, h->x_bn, tiles);
-    h->n_tiles = (int)tiles.size() / 2;
+    h->n_tiles = (int)tiles.size() / 4;
+    std::vector<uint8_t> ptiles;
+    build_pair_tiles(n_inputs, ptiles);
+    h->n_ptiles = (int)ptiles.size() / 4;
+    h->x_pair = want_pair_kernel();
     if ((g_last_error = upload(&h->d_tap_start, tap)) != MWAX_OK ||
+        (g_last_error = upload(&h->d_ptiles, ptiles)) != MWAX_OK ||
         (g_last_error = upload(&h->d_tiles, tiles)) != MWAX_OK) {
         mwax_xcorr_i8_destroy(h); return nullptr;
     }
@@ -564,8 +640,14 @@ int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, vo
     xp.n_inputs = h->n; xp.T = h->n_time; xp.K = h->n_chan; xp.n_out = h->n_chan; xp.n_tiles = h->n_tiles;
     xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = 1; xp.scale = nullptr;
     xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
-    rc = (h->x_bn == 128) ? launch_x<true, 128>(tmap, xp, h->sm_count, (cudaStream_t)stream)
-                          : launch_x<true, 256>(tmap, xp, h->sm_count, (cudaStream_t)stream);
+    if (h->x_pair) {
+        xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
+        rc = launch_x_pair<true>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream);
+        if (rc != MWAX_OK) note_cuda(&h->last_cuda);
+        return rc;
+    }
+    rc = (h->x_bn == 128) ? launch_x<true, 128>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream)
+                          : launch_x<true, 256>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream);
     if (rc != MWAX_OK) note_cuda(&h->last_cuda);
     return rc;
 }
@@ -591,6 +673,7 @@ int mwax_xcorr_i8_destroy(mwax_xcorr_t *h)
     if (!h) return MWAX_OK;
     cudaFree(h->d_tap_start);
     cudaFree(h->d_tiles);
+    cudaFree(h->d_ptiles);
     cudaFree(h->d_in);
     cudaFree(h->d_out);
     delete h;

@@ -64,6 +64,14 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *m, 
         : "memory");
 }
 
+// L2 prefetch of one tensor box (no shared-memory destination, no completion signal)
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap *m, int c0, int c1, int c2)
+{
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(reinterpret_cast<uint64_t>(m)),
+                 "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+
 // ---------------------------------------------------------------- tcgen05
 __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols)
 {
@@ -123,6 +131,142 @@ __device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&r)
         : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// ---------------------------------------------------------------- CTA pairs (cluster of 2, tcgen05 cta_group::2)
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// shared::cluster address of `saddr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
+    return r;
+}
+// arrive on an mbarrier anywhere in the cluster (address from mapa)
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+// TMA load issued by either CTA of a pair: data lands in THIS CTA's shared memory, the transaction bytes are
+// counted on `cluster_bar`, which may live in the other CTA of the pair (the leader's full barrier)
+__device__ __forceinline__ void tma_load_3d_pair(uint32_t dst, const CUtensorMap *m, int c0, int c1, int c2, uint32_t cluster_bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(c0), "r"(c1), "r"(c2), "r"(cluster_bar)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t dst_smem, uint32_t ncols)
+{
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tmem_relinquish_pair()
+{
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr, uint32_t ncols)
+{
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+// commit of the pair's MMAs: one arrival on the mbarrier at this offset in every CTA of `mask`
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar, uint16_t mask)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(bar),
+                 "h"(mask)
+                 : "memory");
+}
+// D[tmem of both CTAs] (+)= A * B^T over the pair: M = 256 (128 rows of A from each CTA), N split in halves
+__device__ __forceinline__ void mma_f16_ss_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                                uint32_t accumulate)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}" ::"r"(
+            d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void mma_i8_ss_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                               uint32_t accumulate)
+{
+    asm volatile(
+        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::2.kind::i8 [%0], %1, %2, %3, p;\n}" ::"r"(
+            d_tmem),
+        "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+
+// ---------------------------------------------------------------- warp-uniform MMA issue
+// One lane of a converged warp, chosen by the hardware.  The MMA warp runs its loops with ALL lanes (so that every
+// operand is warp-uniform and lives in uniform registers) and only the tcgen05 instructions sit behind this
+// predicate; issuing from inside an `if (lane == 0)` region costs ~20 instructions per MMA (R2UR broadcasts and a
+// waterfall loop), which made the issuing thread, not the tensor pipe, the bottleneck.
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t pred;
+    asm volatile("{\n .reg .pred p;\n elect.sync _|p, 0xffffffff;\n selp.u32 %0, 1, 0, p;\n}" : "=r"(pred));
+    return pred != 0;
+}
+// low / high words of the MN-major SWIZZLE_128B descriptor (see make_smem_desc_mn_sw128): the high word is a
+// constant, the low word moves by (bytes >> 4) along the contraction
+__device__ __forceinline__ uint32_t desc_lo(uint32_t smem_addr, uint32_t lbo_bytes)
+{
+    return ((smem_addr & 0x3FFFFu) >> 4) | (((lbo_bytes >> 4) & 0x3FFFu) << 16);
+}
+__host__ __device__ constexpr uint32_t desc_hi(uint32_t sbo_bytes) { return ((sbo_bytes >> 4) & 0x3FFFu) | (1u << 14) | (2u << 29); }
+
+// kind: 0 = f16, 1 = i8; pair: cta_group::2
+template <bool kInt8, bool kPair>
+__device__ __forceinline__ void mma_ss_lohi(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t hi, uint32_t idesc,
+                                            uint32_t accumulate)
+{
+    if (kPair) {
+        if (kInt8)
+            asm volatile("{\n .reg .pred p;\n .reg .b64 da, db;\n setp.ne.b32 p, %5, 0;\n mov.b64 da, {%1, %3};\n mov.b64 db, {%2, %3};\n"
+                         " tcgen05.mma.cta_group::2.kind::i8 [%0], da, db, %4, p;\n}" ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(hi),
+                         "r"(idesc), "r"(accumulate) : "memory");
+        else
+            asm volatile("{\n .reg .pred p;\n .reg .b64 da, db;\n setp.ne.b32 p, %5, 0;\n mov.b64 da, {%1, %3};\n mov.b64 db, {%2, %3};\n"
+                         " tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %4, p;\n}" ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(hi),
+                         "r"(idesc), "r"(accumulate) : "memory");
+    } else {
+        if (kInt8)
+            asm volatile("{\n .reg .pred p;\n .reg .b64 da, db;\n setp.ne.b32 p, %5, 0;\n mov.b64 da, {%1, %3};\n mov.b64 db, {%2, %3};\n"
+                         " tcgen05.mma.cta_group::1.kind::i8 [%0], da, db, %4, p;\n}" ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(hi),
+                         "r"(idesc), "r"(accumulate) : "memory");
+        else
+            asm volatile("{\n .reg .pred p;\n .reg .b64 da, db;\n setp.ne.b32 p, %5, 0;\n mov.b64 da, {%1, %3};\n mov.b64 db, {%2, %3};\n"
+                         " tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %4, p;\n}" ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(hi),
+                         "r"(idesc), "r"(accumulate) : "memory");
+    }
+}
+
+// All the MMAs of one pipeline block (`rows` contraction rows staged at a_src / b_src), issued by the elected lane.
+// KINST rows per instruction = KINST/8 swizzle atoms of 1024 B further along the contraction.
+template <bool kInt8, bool kPair, int BK, int KINST>
+__device__ __forceinline__ void mma_block_issue(uint32_t a_src, uint32_t b_src, uint32_t chunk_bytes, uint32_t d_tmem,
+                                                uint32_t idesc, int rows, uint32_t accumulate)
+{
+    constexpr uint32_t STEP = (KINST / 8) * 1024u / 16u;
+    constexpr uint32_t HI = desc_hi(1024);
+    const uint32_t a_lo = desc_lo(a_src, chunk_bytes), b_lo = desc_lo(b_src, chunk_bytes);
+    if (rows == BK) {
+#pragma unroll
+        for (int ks = 0; ks < BK / KINST; ++ks)
+            mma_ss_lohi<kInt8, kPair>(d_tmem, a_lo + ks * STEP, b_lo + ks * STEP, HI, idesc, ks == 0 ? accumulate : 1u);
+    } else {
+        const int ksteps = (rows + KINST - 1) / KINST;     // rows past the end are TMA zero fill
+        for (int ks = 0; ks < ksteps; ++ks)
+            mma_ss_lohi<kInt8, kPair>(d_tmem, a_lo + ks * STEP, b_lo + ks * STEP, HI, idesc, ks == 0 ? accumulate : 1u);
+    }
+}
 
 // ---------------------------------------------------------------- descriptors
 // Shared-memory matrix descriptor for an MN-major operand stored as TMA writes it with SWIZZLE_128B:

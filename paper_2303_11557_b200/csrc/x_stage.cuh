@@ -28,7 +28,7 @@ struct XParams {
     int K;              // fine channels in Z (taps are taken cyclically mod K)
     int n_out;          // C output channels
     int n_tiles;        // lower-triangle G tiles per channel
-    const uint8_t *tiles;     // [n_tiles][2] = (mi, nj), device
+    const uint8_t *tiles;     // [n_tiles][4] = (mi, nj, w, 0): G rows 128 mi.., G columns 128 nj.. of width 128 w; device
     const int *tap_start;     // [C] first fine-channel position of output channel c
     int n_taps;               // taps per output channel (fine channels summed into one output)
     const float *scale;       // [C] epilogue scale (float path only)
@@ -58,8 +58,59 @@ struct XConfig {
     static constexpr int THREADS = 192;
 };
 
+// Epilogue of one accumulator tile, run by one warp on its 32 TMEM lanes (G rows 2 i, 2 i + 1 of 16 inputs i from
+// i_base) and `ncc` chunks of 32 G columns (16 inputs j from j_base + 16 cc): tcgen05.ld, the 2 x 2 real -> complex
+// fold, scale, Im(auto) := 0, triangle mask, and stores staged through padded shared memory so that
+// each instruction writes 16 consecutive baselines of two rows.  `stg` = this warp's EPI_STAGE_WORDS floats.
+template <bool kInt8>
+__device__ __forceinline__ void x_epilogue_tile(const XParams &P, float *stg, uint32_t t_row, int c, int i_base, int j_base,
+                                                int ncc, float sc, int lane)
+{
+    const int n = P.n_inputs;
+#pragma unroll 1
+    for (int cc = 0; cc < ncc; ++cc) {
+        const int j0 = j_base + cc * 16;         // first of this chunk's 16 inputs j
+        if (j0 > i_base + 15 || j0 >= n || i_base >= n) continue;   // warp-uniform: nothing below the diagonal
+        uint32_t r[32];
+        ptx::tmem_ld_32x32b_x32(t_row + (uint32_t)(cc * 32), r);
+        ptx::tmem_ld_wait();
+        // even lane (G row 2i): Re = G[2i][2j] + G[2i+1][2j+1]; odd lane (row 2i+1): Im = G[2i+1][2j] - G[2i][2j+1]
+#pragma unroll
+        for (int jj = 0; jj < 16; ++jj) {
+            const uint32_t other = __shfl_xor_sync(0xffffffffu, r[2 * jj + 1], 1);
+            float v;
+            if (kInt8) {
+                const int a = (int)r[2 * jj], b = (int)other;
+                const int w = (lane & 1) ? (a - b) : (a + b);
+                v = __int_as_float(w);
+            } else {
+                const float a = __uint_as_float(r[2 * jj]), b = __uint_as_float(other);
+                v = ((lane & 1) ? (a - b) : (a + b)) * sc;
+            }
+            stg[(lane >> 1) * 34 + 2 * jj + (lane & 1)] = v;
+        }
+        __syncwarp();
+        // coalesced store: two rows (inputs i) x 16 complex per instruction
+        const int jl = lane & 15;
+        const int j = j0 + jl;
+#pragma unroll
+        for (int it = 0; it < 8; ++it) {
+            const int row = 2 * it + (lane >> 4);
+            const int i = i_base + row;
+            float2 v = *reinterpret_cast<const float2 *>(&stg[row * 34 + 2 * jl]);
+            if (i < n && j <= i) {
+                if (i == j) v.y = 0.0f;       // autos: Im := 0 exactly (int path: bit pattern 0 as well)
+                const long long o = (long long)c * P.out_chan_stride + ((long long)i * (i + 1) / 2 + j);
+                reinterpret_cast<float2 *>(P.out)[o] = v;
+            }
+        }
+        __syncwarp();
+    }
+}
+
 template <bool kInt8, int BN>
-__global__ void __launch_bounds__(192, 1) x_stage_kernel(const __grid_constant__ CUtensorMap tmap, const XParams P)
+__global__ void __launch_bounds__(192, 1) x_stage_kernel(const __grid_constant__ CUtensorMap tmap,
+                                                         const __grid_constant__ CUtensorMap tmap_flat, const XParams P)
 {
     using C = XConfig<kInt8, BN>;
     extern __shared__ uint8_t smem_raw[];
@@ -84,6 +135,7 @@ __global__ void __launch_bounds__(192, 1) x_stage_kernel(const __grid_constant__
 
     if (warp == 0 && lane == 0) {
         ptx::prefetch_tensormap(&tmap);
+        ptx::prefetch_tensormap(&tmap_flat);
         for (int s = 0; s < C::STAGES; ++s) {
             ptx::mbar_init(full_bar(s), 1);
             ptx::mbar_init(empty_bar(s), 1);
@@ -106,72 +158,101 @@ __global__ void __launch_bounds__(192, 1) x_stage_kernel(const __grid_constant__
     const int n_items = P.n_out * P.n_tiles;
     const int kb_per_tap = (P.T + C::BK - 1) / C::BK;
 
+    // K-loop schedule of one work item (identical in the producer and the MMA issuer).  The taps of an output
+    // channel are adjacent channel positions, i.e. ADJACENT ROWS of Y[p][t]: when T >= BK the contraction runs over
+    // the flattened rows (p T + t) in whole BK-row blocks through `tmap_flat`, so only the END of a run is a partial
+    // block (C4: 51 taps x 200 rows = 159 blocks + 24 rows instead of 51 x (3 blocks + 8 rows)).  The partial block is
+    // fetched through the per-channel map, whose rows past T read as zero.  A tap window that wraps past K (cyclic
+    // taps, Q8) is two runs.
+    const bool flat = (P.n_taps > 1) && (P.T >= C::BK);
+
     if (warp == 0) {
         // ------------------------------------------------------------------ TMA producer
         if (lane == 0) {
             int s = 0;
             uint32_t ph = 0;
+            auto load_block = [&](const CUtensorMap *m, int mi, int nj, int bch, int row, int chan) {
+                ptx::mbar_wait(empty_bar(s), ph ^ 1u);
+                ptx::mbar_arrive_expect_tx(full_bar(s), (uint32_t)(C::A_BYTES + bch * C::CHUNK_BYTES));
+                const uint32_t a_dst = stage_base + s * C::STAGE_BYTES;
+                const uint32_t b_dst = a_dst + C::A_BYTES;
+#pragma unroll
+                for (int ch = 0; ch < C::A_CHUNKS; ++ch)
+                    ptx::tma_load_3d(a_dst + ch * C::CHUNK_BYTES, m, mi * C::BM + ch * C::CHUNK_ELEMS, row, chan, full_bar(s));
+                for (int ch = 0; ch < bch; ++ch)
+                    ptx::tma_load_3d(b_dst + ch * C::CHUNK_BYTES, m, nj * 128 + ch * C::CHUNK_ELEMS, row, chan, full_bar(s));
+                if (++s == C::STAGES) { s = 0; ph ^= 1u; }
+            };
             for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
                 const int c = item / P.n_tiles;
                 const int tile = item - c * P.n_tiles;
-                const int mi = P.tiles[2 * tile], nj = P.tiles[2 * tile + 1];
+                const int mi = P.tiles[4 * tile], nj = P.tiles[4 * tile + 1];
+                const int bch = P.tiles[4 * tile + 2] * (128 / C::CHUNK_ELEMS);   // 128-byte B chunks of this tile
                 const int p0 = P.tap_start[c];
-                for (int tap = 0; tap < P.n_taps; ++tap) {
-                    int p = p0 + tap;
-                    if (p >= P.K) p -= P.K;
-                    for (int kb = 0; kb < kb_per_tap; ++kb) {
-                        ptx::mbar_wait(empty_bar(s), ph ^ 1u);
-                        ptx::mbar_arrive_expect_tx(full_bar(s), C::STAGE_BYTES);
-                        const uint32_t a_dst = stage_base + s * C::STAGE_BYTES;
-                        const uint32_t b_dst = a_dst + C::A_BYTES;
-#pragma unroll
-                        for (int ch = 0; ch < C::A_CHUNKS; ++ch)
-                            ptx::tma_load_3d(a_dst + ch * C::CHUNK_BYTES, &tmap, mi * C::BM + ch * C::CHUNK_ELEMS,
-                                             kb * C::BK, p, full_bar(s));
-#pragma unroll
-                        for (int ch = 0; ch < C::B_CHUNKS; ++ch)
-                            ptx::tma_load_3d(b_dst + ch * C::CHUNK_BYTES, &tmap, nj * BN + ch * C::CHUNK_ELEMS,
-                                             kb * C::BK, p, full_bar(s));
-                        if (++s == C::STAGES) { s = 0; ph ^= 1u; }
+                if (flat) {
+                    const int n1 = min(P.n_taps, P.K - p0);
+                    for (int run = 0; run < 2; ++run) {
+                        const int pf = run ? 0 : p0, nt = run ? P.n_taps - n1 : n1;
+                        if (nt <= 0) continue;
+                        const int rows = nt * P.T, nfull = rows / C::BK, tail = rows - nfull * C::BK;
+                        for (int q = 0; q < nfull; ++q) load_block(&tmap_flat, mi, nj, bch, pf * P.T + q * C::BK, 0);
+                        if (tail) load_block(&tmap, mi, nj, bch, P.T - tail, pf + nt - 1);
+                    }
+                } else {
+                    for (int tap = 0; tap < P.n_taps; ++tap) {
+                        int p = p0 + tap;
+                        if (p >= P.K) p -= P.K;
+                        for (int kb = 0; kb < kb_per_tap; ++kb) load_block(&tmap, mi, nj, bch, kb * C::BK, p);
                     }
                 }
             }
         }
     } else if (warp == 1) {
-        // ------------------------------------------------------------------ MMA issuer (one thread)
-        if (lane == 0) {
+        // ------------------------------------------------------------------ MMA issuer (the whole warp runs the loops so
+        // that every operand is warp-uniform, one elected lane issues: see ptx::elect_one)
+        {
             int s = 0;
             uint32_t ph = 0;
             int as = 0;
             uint32_t aph = 0;
+            uint32_t d_tmem = 0, idesc = 0, accumulate = 0;
+            auto mma_block = [&](int rows) {
+                ptx::mbar_wait(full_bar(s), ph);
+                ptx::tc_fence_after();
+                const uint32_t a_src = stage_base + s * C::STAGE_BYTES;
+                if (ptx::elect_one()) {
+                    ptx::mma_block_issue<kInt8, false, C::BK, C::KINST>(a_src, a_src + C::A_BYTES, C::CHUNK_BYTES, d_tmem, idesc, rows,
+                                                                         accumulate);
+                    ptx::tc_commit(empty_bar(s));       // frees the smem slot when these MMAs have read it
+                }
+                __syncwarp();
+                accumulate = 1;
+                if (++s == C::STAGES) { s = 0; ph ^= 1u; }
+            };
             for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+                const int c = item / P.n_tiles;
+                const int tile = item - c * P.n_tiles;
                 ptx::mbar_wait(tempty_bar(as), aph ^ 1u);
                 ptx::tc_fence_after();
-                const uint32_t d_tmem = tmem_base + (uint32_t)(as * BN);
-                uint32_t accumulate = 0;
-                for (int tap = 0; tap < P.n_taps; ++tap) {
-                    for (int kb = 0; kb < kb_per_tap; ++kb) {
-                        int rows = P.T - kb * C::BK;
-                        if (rows > C::BK) rows = C::BK;
-                        const int ksteps = (rows + C::KINST - 1) / C::KINST;   // rows past T are TMA zero fill
-                        ptx::mbar_wait(full_bar(s), ph);
-                        ptx::tc_fence_after();
-                        const uint32_t a_src = stage_base + s * C::STAGE_BYTES;
-                        const uint32_t b_src = a_src + C::A_BYTES;
-                        for (int ks = 0; ks < ksteps; ++ks) {
-                            // KINST rows = KINST/8 swizzle atoms of 1024 B further along the contraction
-                            const uint32_t koff = (uint32_t)ks * (C::KINST / 8) * 1024u;
-                            const uint64_t a_desc = ptx::make_smem_desc_mn_sw128(a_src + koff, C::CHUNK_BYTES, 1024);
-                            const uint64_t b_desc = ptx::make_smem_desc_mn_sw128(b_src + koff, C::CHUNK_BYTES, 1024);
-                            if (kInt8) ptx::mma_i8_ss(d_tmem, a_desc, b_desc, C::IDESC, accumulate);
-                            else ptx::mma_f16_ss(d_tmem, a_desc, b_desc, C::IDESC, accumulate);
-                            accumulate = 1;
-                        }
-                        ptx::tc_commit(empty_bar(s));   // frees the smem slot when these MMAs have read it
-                        if (++s == C::STAGES) { s = 0; ph ^= 1u; }
+                d_tmem = tmem_base + (uint32_t)(as * BN);
+                idesc = ptx::make_idesc(kInt8 ? 2u : 1u, kInt8 ? 1u : 0u, C::BM, 128u * P.tiles[4 * tile + 2]);
+                accumulate = 0;
+                if (flat) {
+                    const int p0 = P.tap_start[c];
+                    const int n1 = min(P.n_taps, P.K - p0);
+                    for (int run = 0; run < 2; ++run) {
+                        const int nt = run ? P.n_taps - n1 : n1;
+                        if (nt <= 0) continue;
+                        const int rows = nt * P.T, nfull = rows / C::BK, tail = rows - nfull * C::BK;
+                        for (int q = 0; q < nfull; ++q) mma_block(C::BK);
+                        if (tail) mma_block(tail);
                     }
+                } else {
+                    for (int tap = 0; tap < P.n_taps; ++tap)
+                        for (int kb = 0; kb < kb_per_tap; ++kb) mma_block(min(C::BK, P.T - kb * C::BK));
                 }
-                ptx::tc_commit(tfull_bar(as));          // accumulator complete -> epilogue
+                if (ptx::elect_one()) ptx::tc_commit(tfull_bar(as));          // accumulator complete -> epilogue
+                __syncwarp();
                 if (++as == C::ACC_STAGES) { as = 0; aph ^= 1u; }
             }
         }
@@ -181,55 +262,16 @@ __global__ void __launch_bounds__(192, 1) x_stage_kernel(const __grid_constant__
         float *stg = epi_stage + (warp - 2) * C::EPI_STAGE_WORDS;
         int as = 0;
         uint32_t aph = 0;
-        const int n = P.n_inputs;
         for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
             const int c = item / P.n_tiles;
             const int tile = item - c * P.n_tiles;
-            const int mi = P.tiles[2 * tile], nj = P.tiles[2 * tile + 1];
+            const int mi = P.tiles[4 * tile], nj = P.tiles[4 * tile + 1], ncc = 4 * P.tiles[4 * tile + 2];
             const int i_base = mi * (C::BM / 2) + q * 16;       // first input of this warp's 16
             const float sc = kInt8 ? 1.0f : P.scale[c];
             ptx::mbar_wait(tfull_bar(as), aph);
             ptx::tc_fence_after();
             const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * BN);
-#pragma unroll 1
-            for (int cc = 0; cc < BN / 32; ++cc) {
-                const int j0 = nj * (BN / 2) + cc * 16;         // first of this chunk's 16 inputs j
-                if (j0 > i_base + 15 || j0 >= n || i_base >= n) continue;   // warp-uniform: nothing below the diagonal
-                uint32_t r[32];
-                ptx::tmem_ld_32x32b_x32(t_row + (uint32_t)(cc * 32), r);
-                ptx::tmem_ld_wait();
-                // even lane (G row 2i): Re = G[2i][2j] + G[2i+1][2j+1]; odd lane (row 2i+1): Im = G[2i+1][2j] - G[2i][2j+1]
-#pragma unroll
-                for (int jj = 0; jj < 16; ++jj) {
-                    const uint32_t other = __shfl_xor_sync(0xffffffffu, r[2 * jj + 1], 1);
-                    float v;
-                    if (kInt8) {
-                        const int a = (int)r[2 * jj], b = (int)other;
-                        const int w = (lane & 1) ? (a - b) : (a + b);
-                        v = __int_as_float(w);
-                    } else {
-                        const float a = __uint_as_float(r[2 * jj]), b = __uint_as_float(other);
-                        v = ((lane & 1) ? (a - b) : (a + b)) * sc;
-                    }
-                    stg[(lane >> 1) * 34 + 2 * jj + (lane & 1)] = v;
-                }
-                __syncwarp();
-                // coalesced store: two rows (inputs i) x 16 complex per instruction
-                const int jl = lane & 15;
-                const int j = j0 + jl;
-#pragma unroll
-                for (int it = 0; it < 8; ++it) {
-                    const int row = 2 * it + (lane >> 4);
-                    const int i = i_base + row;
-                    float2 v = *reinterpret_cast<const float2 *>(&stg[row * 34 + 2 * jl]);
-                    if (i < n && j <= i) {
-                        if (i == j) v.y = 0.0f;       // autos: Im := 0 exactly (int path: bit pattern 0 as well)
-                        const long long o = (long long)c * P.out_chan_stride + ((long long)i * (i + 1) / 2 + j);
-                        reinterpret_cast<float2 *>(P.out)[o] = v;
-                    }
-                }
-                __syncwarp();
-            }
+            x_epilogue_tile<kInt8>(P, stg, t_row, c, i_base, nj * 64, ncc, sc, lane);
             ptx::tc_fence_before();
             __syncwarp();
             if (lane == 0) ptx::mbar_arrive(tempty_bar(as));
