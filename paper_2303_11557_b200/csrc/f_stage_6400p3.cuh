@@ -102,13 +102,18 @@ __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster
 // relaxed arrive: orders nothing; enough to tell the other CTAs "I have finished READING your shared memory"
 __device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
-// 16 bytes from the shared memory of CTA `rank` of this cluster, at the same offset as local address `saddr`
-__device__ __forceinline__ uint4 ld_dsmem_v4(uint32_t saddr, uint32_t rank)
+// shared::cluster address of local shared address `saddr` in CTA `rank` of this cluster
+__device__ __forceinline__ uint32_t ld_dsmem_base(uint32_t saddr, uint32_t rank)
 {
     uint32_t ra;
-    uint4 v;
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(saddr), "r"(rank));
-    asm volatile("ld.shared::cluster.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(ra) : "memory");
+    return ra;
+}
+// 16 bytes from distributed shared memory
+__device__ __forceinline__ uint4 ld_shared_cluster_v4(uint32_t caddr)
+{
+    uint4 v;
+    asm volatile("ld.shared::cluster.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(caddr) : "memory");
     return v;
 }
 
@@ -265,21 +270,41 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
         cluster_wait();                                              // every CTA of the cluster has staged its rows
 
         // ---- corner-turned store: this CTA writes rows k3 in [rank 16/Q, (rank + 1) 16/Q) for all 4 Q inputs
-        const uint32_t s_base = (uint32_t)__cvta_generic_to_shared(esm);
-#pragma unroll 2
-        for (int it = 0; it < (C::N / C::THREADS); ++it) {
-            const int u = threadIdx.x + C::THREADS * it;
-            const int q = u % Q, rowid = u / Q;
-            const int kl = rowid / 400, c = rowid - 400 * kl;
-            const int k3 = (int)rank * (16 / Q) + kl;
-            const int k2 = c / 20, k1 = c - 20 * k2;
-            const uint32_t sa = s_base + (uint32_t)(((k3 < 8 ? 0 : 3 * C::SG) + k1 * C::S1 + k2 * 16) * 8 + (k3 & 7) * 16);
-            const uint4 v = ld_dsmem_v4(sa, (uint32_t)q);
+        // Thread = (piece q = tid % Q of a row, row stream tid / Q + (640 / Q) it): 640 / Q is a multiple of 20, so k1 is
+        // a per-thread constant and (c, k3) advance by additions.  Loads go out in batches of 4 (all of a batch's
+        // remote reads in flight together), then the batch is stored: 16-byte pieces, Q adjacent lanes per row.
+        {
+            constexpr int RSTEP = C::THREADS / Q;                    // rows per iteration (320 / 160 / 80)
+            const int q = threadIdx.x % Q;
+            const uint32_t rbase = ld_dsmem_base((uint32_t)__cvta_generic_to_shared(esm), (uint32_t)q);
             const int col = (grp * Q + q) * C::G;
-            const int k = c + 400 * k3;
-            const int p = ((k < C::N / 2) ? k : k - C::N) + half;    // centre order; keep (L611)
-            if (col < P.pitch2 && (FULL || (p >= 0 && p < P.K)))
-                *reinterpret_cast<uint4 *>(P.Y + (size_t)p * chan_stride + (size_t)t * P.y_t_stride + col) = v;
+            const bool col_ok = col < P.pitch2;
+            __half2 *ycol = P.Y + (size_t)t * P.y_t_stride + col;
+            int c = threadIdx.x / Q, kl = 0;
+            const int k1 = c % 20;
+            constexpr int NB = 4;                                    // loads in flight per thread
+#pragma unroll 1
+            for (int b0 = 0; b0 < C::N / C::THREADS; b0 += NB) {
+                uint4 pv[NB];
+                int pk[NB];
+#pragma unroll
+                for (int e = 0; e < NB; ++e) {
+                    if (b0 + e >= C::N / C::THREADS) break;
+                    const int k3 = (int)rank * (16 / Q) + kl;
+                    const int k2 = c / 20;
+                    const uint32_t so = (uint32_t)(((k3 < 8 ? 0 : 3 * C::SG) + k1 * C::S1 + k2 * 16) * 8 + (k3 & 7) * 16);
+                    pv[e] = ld_shared_cluster_v4(rbase + so);
+                    pk[e] = c + 400 * k3;
+                    c += RSTEP;
+                    if (c >= 400) { c -= 400; ++kl; }
+                }
+#pragma unroll
+                for (int e = 0; e < NB; ++e) {
+                    if (b0 + e >= C::N / C::THREADS) break;
+                    const int p = ((pk[e] < C::N / 2) ? pk[e] : pk[e] - C::N) + half;   // centre order (L290); keep (L611)
+                    if (col_ok && (FULL || (p >= 0 && p < P.K))) *reinterpret_cast<uint4 *>(ycol + (size_t)p * chan_stride) = pv[e];
+                }
+            }
         }
         cluster_arrive_relaxed();                                    // pairs with the wait inside the next pass 1
     }
