@@ -246,15 +246,18 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
             uint32_t *s_lo = reinterpret_cast<uint32_t *>(esm + slot) + g;
             uint32_t *s_hi = reinterpret_cast<uint32_t *>(esm + 3 * C::SG + slot) + g;
             const uint32_t code = (FULL && SCALE) ? codes[c] : 0u;   // 2 bits per k3: 0 -> 1, 1 -> sqrt(1/2), 2 -> 0
+            if (FULL && SCALE && code != 0u) {                       // rare: 8 + 1 of the 400 tasks at F = 50
+#pragma unroll
+                for (int k3 = 0; k3 < 16; ++k3) {
+                    const uint32_t cd = (code >> (2 * k3)) & 3u;
+                    const float f = cd == 0u ? 1.0f : (cd == 1u ? 0.70710678118654757f : 0.0f);
+                    z[bitrev(k3, 4)].x *= f;
+                    z[bitrev(k3, 4)].y *= f;
+                }
+            }
 #pragma unroll
             for (int k3 = 0; k3 < 16; ++k3) {
                 float2 v = z[bitrev(k3, 4)];
-                if (FULL && SCALE) {
-                    const uint32_t cd = (code >> (2 * k3)) & 3u;
-                    const float f = cd == 0u ? 1.0f : (cd == 1u ? 0.70710678118654757f : 0.0f);
-                    v.x *= f;
-                    v.y *= f;
-                }
                 if (!FULL && SCALE) {
                     const int k = c + 400 * k3;
                     const int p = ((k < C::N / 2) ? k : k - C::N) + half;

@@ -270,6 +270,9 @@ struct mwax_corr {
     size_t in_bytes;
     float *d_out;
     size_t out_bytes;
+    cudaStream_t s_in, s_out;              // copy streams of process_host
+    cudaEvent_t ev_start, ev_copied;
+    std::vector<cudaEvent_t> ev_in, ev_done;
 };
 
 struct mwax_xcorr {
@@ -550,9 +553,11 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
     if (!h || !h_volt || !h_vis) return MWAX_ERR_NULL;
     if (n_dumps < 1 || n_coarse < 1 || row_pitch < (size_t)n_dumps * h->T * h->N) return MWAX_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t row_samples = (size_t)n_dumps * h->T * h->N;
+    const size_t dump_samples = (size_t)h->T * h->N;
+    const size_t row_samples = (size_t)n_dumps * dump_samples;
     const size_t in_bytes = (size_t)h->n * row_samples * 2;
-    const size_t out_bytes = (size_t)n_dumps * mwax_corr_output_bytes(h);
+    const size_t dump_out = mwax_corr_output_bytes(h);
+    const size_t out_bytes = (size_t)n_dumps * dump_out;
     if (h->in_bytes < in_bytes) {
         cudaFree(h->d_in); h->d_in = nullptr; h->in_bytes = 0;
         if (cudaMalloc(reinterpret_cast<void **>(&h->d_in), in_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
@@ -563,16 +568,55 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
         if (cudaMalloc(reinterpret_cast<void **>(&h->d_out), out_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
         h->out_bytes = out_bytes;
     }
-    for (int c = 0; c < n_coarse; ++c) {
-        if (cudaMemcpy2DAsync(h->d_in, row_samples * 2, h_volt + 2 * c * coarse_pitch, row_pitch * 2, row_samples * 2,
-                              h->n, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    // Three streams so that PCIe runs in both directions under the kernels: dump d + 1 travels host -> device and
+    // dump d - 1 device -> host while dump d is correlated on the caller's stream.
+    if (!h->s_in && cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking) != cudaSuccess) return note_cuda(&h->last_cuda);
+    if (!h->s_out && cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking) != cudaSuccess) return note_cuda(&h->last_cuda);
+    const int n_ev = n_dumps * n_coarse;
+    while ((int)h->ev_in.size() < n_ev) {
+        cudaEvent_t a, b;
+        if (cudaEventCreateWithFlags(&a, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&b, cudaEventDisableTiming) != cudaSuccess)
             return note_cuda(&h->last_cuda);
-        int rc = mwax_corr_process_batch(h, h->d_in, row_samples, 0, n_dumps, 1, h->d_out, st);
-        if (rc != MWAX_OK) return rc;
-        if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c * out_bytes, h->d_out, out_bytes,
-                            cudaMemcpyDeviceToHost, st) != cudaSuccess)
+        h->ev_in.push_back(a);
+        h->ev_done.push_back(b);
+    }
+    if (!h->ev_start) {
+        if (cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->ev_copied, cudaEventDisableTiming) != cudaSuccess)
             return note_cuda(&h->last_cuda);
     }
+    // the copy streams start after whatever the caller has already queued on `stream`
+    cudaEventRecord(h->ev_start, st);
+    cudaStreamWaitEvent(h->s_in, h->ev_start, 0);
+    cudaStreamWaitEvent(h->s_out, h->ev_start, 0);
+    const size_t vis_floats = dump_out / sizeof(float);
+    for (int c = 0; c < n_coarse; ++c)
+        for (int d = 0; d < n_dumps; ++d) {
+            const int e = c * n_dumps + d;
+            // staging is reused by the next coarse channel: its dump d may be overwritten once it has been correlated
+            if (c > 0) cudaStreamWaitEvent(h->s_in, h->ev_done[e - n_dumps], 0);
+            if (cudaMemcpy2DAsync(h->d_in + 2 * d * dump_samples, row_samples * 2,
+                                  h_volt + 2 * (c * coarse_pitch + d * dump_samples), row_pitch * 2, dump_samples * 2, h->n,
+                                  cudaMemcpyHostToDevice, h->s_in) != cudaSuccess)
+                return note_cuda(&h->last_cuda);
+            cudaEventRecord(h->ev_in[e], h->s_in);
+            cudaStreamWaitEvent(st, h->ev_in[e], 0);
+            if (c > 0) cudaStreamWaitEvent(st, h->ev_copied, 0);   // previous channel's visibilities have left d_out
+            int rc = mwax_corr_f_stage(h, h->d_in + 2 * d * dump_samples, row_samples, st);
+            if (rc != MWAX_OK) return rc;
+            rc = mwax_corr_x_stage(h, h->d_out + (size_t)d * vis_floats, st);
+            if (rc != MWAX_OK) return rc;
+            cudaEventRecord(h->ev_done[e], st);
+            cudaStreamWaitEvent(h->s_out, h->ev_done[e], 0);
+            if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c * out_bytes + (size_t)d * dump_out,
+                                h->d_out + (size_t)d * vis_floats, dump_out, cudaMemcpyDeviceToHost, h->s_out) != cudaSuccess)
+                return note_cuda(&h->last_cuda);
+            if (d == n_dumps - 1) cudaEventRecord(h->ev_copied, h->s_out);
+        }
+    // join: the caller's stream continues after the last copy; the call itself returns when everything has landed
+    cudaEventRecord(h->ev_copied, h->s_out);
+    cudaStreamWaitEvent(st, h->ev_copied, 0);
     if (cudaStreamSynchronize(st) != cudaSuccess) return note_cuda(&h->last_cuda);
     return MWAX_OK;
 }
@@ -594,6 +638,12 @@ int mwax_corr_destroy(mwax_corr_t *h)
     cudaFree(h->d_Y);
     cudaFree(h->d_in);
     cudaFree(h->d_out);
+    for (cudaEvent_t e : h->ev_in) cudaEventDestroy(e);
+    for (cudaEvent_t e : h->ev_done) cudaEventDestroy(e);
+    if (h->ev_start) cudaEventDestroy(h->ev_start);
+    if (h->ev_copied) cudaEventDestroy(h->ev_copied);
+    if (h->s_in) cudaStreamDestroy(h->s_in);
+    if (h->s_out) cudaStreamDestroy(h->s_out);
     delete h;
     return MWAX_OK;
 }
