@@ -207,6 +207,35 @@ int mwax_oracle_spectra(int n_sel, const int *sel, int N, int K, int T, int dump
     return err;
 }
 
+/* Step 3b (PAPER.md 2.5.1 L266-272, 2.4.1 L221, 4.3 L585): fractional-delay / phase
+ * correction.  "any remaining fractional sample delay components can be applied by multiplying the frequency-domain
+ * samples of each signal path by a phase gradient ... gradients can differ in both their slope and phase offset.
+ * The slopes depend only on the delays to be applied, while the phase offsets [are supplied per path]"; one value
+ * per signal path per frame ("5 ms update rate", 1600 values per 8 s at N = 6400).  Reading Q19:
+ * APPLYING a delay of d samples to a signal multiplies bin u of its spectrum by exp(-2 pi i u d / N) (shift
+ * theorem, forward transform of reading Q1); the phase offset phi (radians) multiplies by exp(+i phi):
+ *     Y[p][t][s] *= exp(i * (phase[i][f] - 2 pi u d[i][f] / N)),  u = p - floor(K/2),  i = sel[s],  f = dump*T + t.
+ * The paper takes the gains from a pre-computed look-up table; here they are computed directly (cos/sin in double).
+ * delay, phase: [n_inputs][row_stride] doubles (NULL = all zero). */
+int mwax_oracle_apply_delays(int n_sel, const int *sel, int N, int K, int T, int dump, const double *delay,
+                             const double *phase, int64_t row_stride, double *Y_ri)
+{
+    if (n_sel < 1 || !sel || N < 1 || K < 1 || K > N || T < 1 || dump < 0 || !Y_ri) return ORACLE_ERR_ARG;
+    cplx *Y = (cplx *)Y_ri;
+#pragma omp parallel for schedule(static)
+    for (int p = 0; p < K; ++p) {
+        const int u = p - K / 2;
+        for (int t = 0; t < T; ++t)
+            for (int s = 0; s < n_sel; ++s) {
+                const int64_t o = (int64_t)sel[s] * row_stride + (int64_t)dump * T + t;
+                const double d = delay ? delay[o] : 0.0, ph = phase ? phase[o] : 0.0;
+                const double th = ph - TWO_PI * (double)u * d / (double)N;
+                Y[((size_t)p * T + t) * n_sel + s] *= cos(th) + I * sin(th);
+            }
+    }
+    return ORACLE_OK;
+}
+
 /* Step 4: R[p][a(a+1)/2 + b] = sum_{t<T} Y_a[p][t] * conj(Y_b[p][t]) for all a >= b (autos included):
  * "cross-multiply every input pair", summed (not averaged) over the integration
  * (L280; reading Q5).  Direct per-pair multiply-accumulate.  Reading Q2: the SECOND index is conjugated. */
@@ -265,9 +294,11 @@ int mwax_oracle_average(int n_sel, int K, int F, int mode, const double *R_ri, d
 }
 
 /* Whole float path for one dump and a selection of inputs (steps 1-6 in order).
- * vis: [C][n_sel(n_sel+1)/2][re,im] float64; pair (a,b), a >= b, refers to inputs sel[a], sel[b]. */
-int mwax_oracle_fx(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,
-                   const int8_t *volt, int64_t row_pitch, double *vis_ri)
+ * vis: [C][n_sel(n_sel+1)/2][re,im] float64; pair (a,b), a >= b, refers to inputs sel[a], sel[b].
+ * The _delay form inserts step 3b between steps 3 and 4. */
+int mwax_oracle_fx_delay(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,
+                         const int8_t *volt, int64_t row_pitch, const double *delay, const double *phase,
+                         int64_t row_stride, double *vis_ri)
 {
     if (n_sel < 1 || K < 1 || F < 1 || K % F != 0 || T < 1) return ORACLE_ERR_ARG;
     const size_t B = (size_t)n_sel * (n_sel + 1) / 2;
@@ -275,11 +306,19 @@ int mwax_oracle_fx(int n_sel, const int *sel, int N, int K, int T, int F, int mo
     double *R = (double *)malloc(sizeof(double) * 2 * (size_t)K * B);
     if (!Y || !R) { free(Y); free(R); return ORACLE_ERR_NOMEM; }
     int rc = mwax_oracle_spectra(n_sel, sel, N, K, T, dump, volt, row_pitch, Y);
+    if (rc == ORACLE_OK && (delay || phase))
+        rc = mwax_oracle_apply_delays(n_sel, sel, N, K, T, dump, delay, phase, row_stride, Y);
     if (rc == ORACLE_OK) rc = mwax_oracle_correlate(n_sel, K, T, Y, R);
     if (rc == ORACLE_OK) rc = mwax_oracle_average(n_sel, K, F, mode, R, vis_ri);
     free(Y);
     free(R);
     return rc;
+}
+
+int mwax_oracle_fx(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,
+                   const int8_t *volt, int64_t row_pitch, double *vis_ri)
+{
+    return mwax_oracle_fx_delay(n_sel, sel, N, K, T, F, mode, dump, volt, row_pitch, NULL, NULL, 0, vis_ri);
 }
 
 /* Integer X-only path (BASELINE.json configs[1]; the same contraction as step 4 on pre-channelised int8

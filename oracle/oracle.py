@@ -47,6 +47,10 @@ def _load():
         lib.mwax_oracle_average.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp]
         lib.mwax_oracle_fx.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                        ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp]
+        lib.mwax_oracle_apply_delays.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                 dp, dp, ctypes.c_int64, dp]
+        lib.mwax_oracle_fx_delay.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                             ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp, dp, ctypes.c_int64, dp]
         lib.mwax_oracle_xcorr_i8.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, i8p, i32p]
         lib.mwax_oracle_threads.argtypes = []
         _lib = lib
@@ -121,16 +125,47 @@ def average(R: np.ndarray, n: int, F: int, mode: int = AVG_CENTRE_SYMMETRIC) -> 
     return V
 
 
+def _tab(a, n_inputs):
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    assert a.ndim == 2 and a.shape[0] == n_inputs
+    return a, _dp(a)
+
+
+def apply_delays(Y: np.ndarray, N: int, delay=None, phase=None, dump: int = 0, sel=None, n_inputs=None) -> np.ndarray:
+    """Step 3b: Y complex128 [K][T][n_sel] times exp(i (phase - 2 pi u delay / N)); tables [n_inputs][frames]."""
+    Y = np.array(Y, dtype=np.complex128, order="C")
+    K, T, n_sel = Y.shape
+    n_inputs = n_inputs if n_inputs is not None else (delay if delay is not None else phase).shape[0]
+    s, sp = _sel(sel, n_inputs)
+    assert s.size == n_sel
+    d, dpp = _tab(delay, n_inputs)
+    ph, php = _tab(phase, n_inputs)
+    stride = (d if d is not None else ph).shape[1]
+    assert stride >= (dump + 1) * T and (d is None or ph is None or d.shape == ph.shape)
+    _check(_load().mwax_oracle_apply_delays(n_sel, sp, N, K, T, dump, dpp, php, stride, _dp(Y.view(np.float64))),
+           "apply_delays")
+    return Y
+
+
 def fx(volt: np.ndarray, N: int, K: int, T: int, F: int, mode: int = AVG_CENTRE_SYMMETRIC, dump: int = 0,
-       sel=None) -> np.ndarray:
-    """Whole float path, one dump: int8 [n][samples][2] -> V complex128 [K/F][n_sel(n_sel+1)/2]."""
+       sel=None, delay=None, phase=None) -> np.ndarray:
+    """Whole float path, one dump: int8 [n][samples][2] -> V complex128 [K/F][n_sel(n_sel+1)/2].
+    delay / phase: optional [n][frames] tables of the fractional-delay correction (step 3b)."""
     assert volt.dtype == np.int8 and volt.ndim == 3 and volt.shape[2] == 2 and volt.flags.c_contiguous
     assert volt.shape[1] >= (dump + 1) * T * N
     s, sp = _sel(sel, volt.shape[0])
     V = np.empty((K // F, s.size * (s.size + 1) // 2), dtype=np.complex128)
-    _check(_load().mwax_oracle_fx(s.size, sp, N, K, T, F, mode, dump,
-                                  volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), volt.shape[1],
-                                  _dp(V.view(np.float64))), "fx")
+    d, dpp = _tab(delay, volt.shape[0])
+    ph, php = _tab(phase, volt.shape[0])
+    stride = 0
+    if d is not None or ph is not None:
+        stride = (d if d is not None else ph).shape[1]
+        assert stride >= (dump + 1) * T and (d is None or ph is None or d.shape == ph.shape)
+    _check(_load().mwax_oracle_fx_delay(s.size, sp, N, K, T, F, mode, dump,
+                                        volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), volt.shape[1],
+                                        dpp, php, stride, _dp(V.view(np.float64))), "fx")
     return V
 
 
