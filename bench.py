@@ -266,6 +266,24 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
            "ws_bytes": h.workspace_bytes(), "e2e": None,
            "input_samples_per_s": world * n * row / (ms_per_step * 1e-3)}
 
+    # ---- F stage with the fractional-delay / phase correction switched on
+    g = torch.Generator(device="cuda").manual_seed(1234 + rank)
+    dly = (torch.rand((n, T * D), generator=g, device="cuda") - 0.5).float().contiguous()
+    phs = ((torch.rand((n, T * D), generator=g, device="cuda") - 0.5) * 6.0).float().contiguous()
+    h.set_delays(dly, phs)
+    for _ in range(2):
+        corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr(), row, sp), "f_stage", h._h)
+    d0 = torch.cuda.Event(enable_timing=True)
+    d1 = torch.cuda.Event(enable_timing=True)
+    n_rep = 10
+    d0.record(stream)
+    for _ in range(n_rep):
+        corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr(), row, sp), "f_stage", h._h)
+    d1.record(stream)
+    torch.cuda.synchronize()
+    res["f_ms_delay"] = d0.elapsed_time(d1) / n_rep
+    h.set_delays(None, None)
+
     # ---- e2e through the public host-buffer call (H2D + D2H inside the timed region)
     if do_e2e:
         hvis = torch.empty((1, D, C, B, 2), dtype=torch.float32).pin_memory()
@@ -311,6 +329,7 @@ def rooflines(res, peaks, traffic, wl):
               "executed_over_algorithmic": "tiles cover 1.25x the lower triangle at n=512 (DESIGN.md 5.2)"}
     roof_f = {"kernel": f_name, "bound": "hbm", "achieved": f_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
               "frac": f_ach / peaks["hbm_gbs"], "traffic": traffic.get((wl, "f")), "avg_launch_ms": res["f_ms"],
+              "avg_launch_ms_with_delay_phase_correction": res.get("f_ms_delay"),
               "peak_source": f"{peaks['source']} copy bandwidth (MEASURED_PEAKS.json)"}
     return roof_f, roof_x
 

@@ -70,6 +70,20 @@ int mwax_corr_last_error(void);
 /* Averaging geometry; call before the first process().  Default MWAX_AVG_CENTRE_SYMMETRIC. */
 int mwax_corr_set_option(mwax_corr_t *h, int key, int value);
 
+/* Fractional-delay / phase correction (§2.5.1, §2.4.1, §4.3):
+ * before cross-correlation every signal path's spectrum is multiplied by a phase gradient whose slope is the
+ * fractional-sample delay to apply and by a phase offset, one pair of values per signal path per frame (the paper's
+ * 5 ms cadence: 1600 values per 8 s at n_fft = 6400).  Signed bin u of frame f of input i is multiplied by
+ *     exp(i * (phase[i][f] - 2 pi u delay[i][f] / n_fft))          (delay in samples, phase in radians;
+ * applying a delay of d samples; reading Q19).  The gains are computed in the F kernel (no look-up table).
+ *   d_delay, d_phase  DEVICE float tables, entry (coarse c, input i, frame f) at c*coarse_stride + i*row_stride + f;
+ *                     frame f counts the frames of the row handed to process()/process_batch()/process_host()
+ *                     (dump d uses frames d*T .. d*T+T-1).  Either may be NULL (= zeros); both NULL switches the
+ *                     correction off.  Caller-owned; must stay valid while calls that use them are in flight.
+ *   row_stride >= frames per row (T * n_dumps), else MWAX_ERR_INVALID_ARG (checked again by the process calls). */
+int mwax_corr_set_delays(mwax_corr_t *h, const float *d_delay, const float *d_phase, size_t row_stride,
+                         size_t coarse_stride);
+
 /* One integration:
  *   d_volt  in : int8 [n_inputs][T*N][re,im] — row i is signal path i's contiguous sample stream
  *                (PAPER.md L260), row pitch exactly T*N samples; two's-complement, -128 accepted.

@@ -71,6 +71,7 @@ def lib() -> ctypes.CDLL:
         L.mwax_corr_process_batch.argtypes = [vp, vp, sz, sz, i32, i32, vp, vp]
         L.mwax_corr_process_host.argtypes = [vp, vp, sz, sz, i32, i32, vp, vp]
         L.mwax_corr_f_stage.argtypes = [vp, vp, sz, vp]
+        L.mwax_corr_set_delays.argtypes = [vp, vp, vp, sz, sz]
         L.mwax_corr_x_stage.argtypes = [vp, vp, vp]
         for f in ("input_bytes", "output_bytes", "workspace_bytes"):
             getattr(L, "mwax_corr_" + f).restype = sz
@@ -167,6 +168,23 @@ class MwaxCorr:
                                             n_coarse, vis.data_ptr(), _stream_ptr(stream)),
                "mwax_corr_process_host", self._h)
         return vis
+
+    def set_delays(self, delay: torch.Tensor | None, phase: torch.Tensor | None):
+        """delay (samples) / phase (radians): float32 cuda [n][frames] or [n_coarse][n][frames]; None = zeros; both
+        None switches the correction off.  The tensors are kept alive by this object."""
+        ref = delay if delay is not None else phase
+        if ref is None:
+            self._delay_refs = None
+            _check(lib().mwax_corr_set_delays(self._h, None, None, 0, 0), "mwax_corr_set_delays", self._h)
+            return
+        for t in (delay, phase):
+            assert t is None or (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.shape == ref.shape)
+        assert ref.dim() in (2, 3) and ref.shape[-2] == self.n_inputs
+        row_stride = ref.shape[-1]
+        self._delay_refs = (delay, phase)
+        _check(lib().mwax_corr_set_delays(self._h, delay.data_ptr() if delay is not None else None,
+                                          phase.data_ptr() if phase is not None else None, row_stride,
+                                          row_stride * self.n_inputs), "mwax_corr_set_delays", self._h)
 
     def f_stage(self, volt: torch.Tensor, row_pitch: int | None = None, stream=None):
         assert volt.is_cuda and volt.dtype == torch.int8 and volt.is_contiguous()

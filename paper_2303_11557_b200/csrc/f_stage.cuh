@@ -29,6 +29,12 @@ struct FParams {
     const float *sw;         // [K] per-position factor sqrt(w_p): 1, sqrt(1/2) on a shared edge, 0 for excluded DC
     float in_scale;          // s: power-of-two F-stage scale (keeps fp16 in range)
     int chan_scale;          // 0 when every sw[p] == 1
+    // fractional-delay / phase correction (PAPER.md 2.5.1 L266-272): entry (input i, frame f) at i * d_stride + f; the
+    // kernel's frame t is table frame frame0 + t.  NULL = zero.  Applied only by the DELAY kernel variants.
+    const float *delay;      // samples
+    const float *phase;      // radians
+    long long d_stride;
+    int frame0;
     __half2 *Y;              // [K][T][pitch2]
     int pitch2;              // half2 (complex) elements per Y row
     unsigned y_p_stride, y_t_stride;   // half2 elements between channel positions / between spectra (p3 kernel)
@@ -37,6 +43,28 @@ struct FParams {
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 {
     return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+
+// Delay/phase gain of one (input, frame): applying a delay of d samples multiplies signed bin u by
+// exp(i (phase - 2 pi u d / N)) (shift theorem; reading Q19).  Kept in TURNS so that the argument of the
+// fast sine/cosine is reduced exactly: turns(u) = pt + u * st, pt = phase / 2 pi, st = -d / N.
+struct DelayGain {
+    float pt, st;
+};
+__device__ __forceinline__ DelayGain load_delay_gain(const float *delay, const float *phase, long long idx, float inv_n)
+{
+    DelayGain gn;
+    gn.pt = phase ? __ldg(phase + idx) * 0.15915494309189535f : 0.0f;
+    gn.st = delay ? -__ldg(delay + idx) * inv_n : 0.0f;
+    return gn;
+}
+__device__ __forceinline__ float2 apply_delay_gain(float2 v, DelayGain gn, int u)
+{
+    float tr = fmaf((float)u, gn.st, gn.pt);
+    tr -= rintf(tr);                                                 // [-0.5, 0.5] turns
+    float sn, cs;
+    __sincosf(tr * 6.283185307179586f, &sn, &cs);
+    return make_float2(fmaf(v.x, cs, -v.y * sn), fmaf(v.x, sn, v.y * cs));
 }
 
 // y_k = sum_j x_j w_R^{jk}, forward (w_R = exp(-2 pi i / R))
@@ -168,7 +196,10 @@ __global__ void __launch_bounds__(256) f_stage_generic_kernel(const FParams P)
         int k = p - half;
         if (k < 0) k += N;
         const float f = __ldg(&P.sw[p]) * P.in_scale;
-        const float2 v = src[k * G + g];
+        float2 v = src[k * G + g];
+        if (P.delay || P.phase)
+            v = apply_delay_gain(v, load_delay_gain(P.delay, P.phase, (long long)i * P.d_stride + P.frame0 + t, 1.0f / (float)N),
+                                 p - half);
         P.Y[((long long)p * P.T + t) * P.pitch2 + i] = __floats2half2_rn(v.x * f, v.y * f);
     }
 }

@@ -124,7 +124,8 @@ __device__ __forceinline__ uint4 ld_shared_cluster_v4(uint32_t caddr)
 //        16 Q contiguous bytes at once (Q = 2: whole 32-byte sectors, Q = 8: whole 128-byte lines).  With one CTA
 //        per row piece (Q = 1) the 16-byte pieces of a sector arrive from different SMs at different times and L2
 //        turns them into read-modify-write DRAM traffic (ncu: profiles/r1_f6400.md).
-template <bool FULL, bool SCALE, int Q>
+// DELAY: fractional-delay / phase gain per (input, frame) applied to the pass-3 results (PAPER.md 2.5.1 L266-272)
+template <bool FULL, bool SCALE, int Q, bool DELAY = false>
 __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(const FParams P)
 {
     using C = F6400P3;
@@ -229,6 +230,12 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
         // the next item's voltages travel while pass 3 computes and stores
         fetch(item + item_step);
 
+        DelayGain gn = {0.f, 0.f};
+        if (DELAY) {
+            const int i = (grp * Q + (int)rank) * C::G + g;
+            if (i < P.n_inputs) gn = load_delay_gain(P.delay, P.phase, (long long)i * P.d_stride + P.frame0 + t, 1.0f / (float)C::N);
+        }
+
         // ---- pass 3: tasks c = k1 + 20 k2 = j + 160 r: 16-point FFT over n3 -> bins k = c + 400 k3, rounded to fp16 and
         // staged in place as rows S(c, k3) = 4 inputs x 4 bytes, inside the slots of inputs 0 (k3 < 8) and 3 (k3 >= 8)
 #pragma unroll 1
@@ -246,6 +253,11 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
             uint32_t *s_lo = reinterpret_cast<uint32_t *>(esm + slot) + g;
             uint32_t *s_hi = reinterpret_cast<uint32_t *>(esm + 3 * C::SG + slot) + g;
             const uint32_t code = (FULL && SCALE) ? codes[c] : 0u;   // 2 bits per k3: 0 -> 1, 1 -> sqrt(1/2), 2 -> 0
+            if (DELAY) {
+#pragma unroll
+                for (int k3 = 0; k3 < 16; ++k3)
+                    z[bitrev(k3, 4)] = apply_delay_gain(z[bitrev(k3, 4)], gn, c + 400 * k3 - (k3 < 8 ? 0 : C::N));
+            }
             if (FULL && SCALE && code != 0u) {                       // rare: 8 + 1 of the 400 tasks at F = 50
 #pragma unroll
                 for (int k3 = 0; k3 < 16; ++k3) {

@@ -109,7 +109,8 @@ struct FPow2Config {
 };
 
 // FULL : K == N (every bin is kept; no range checks)          SCALE : multiply by sw[p] (averaging weights)
-template <int N, int R1, int PTS, bool FULL, bool SCALE>
+// DELAY: fractional-delay / phase gain per (input, frame) (PAPER.md 2.5.1 L266-272)
+template <int N, int R1, int PTS, bool FULL, bool SCALE, bool DELAY = false>
 __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2_kernel(const FParams P)
 {
     using C = FPow2Config<N, R1, PTS>;
@@ -231,6 +232,8 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
         }
         __syncthreads();                                              // ex complete; raw(t) no longer needed
         if (more) stash(q);
+        DelayGain gn = {0.f, 0.f};
+        if (DELAY && iok) gn = load_delay_gain(P.delay, P.phase, (long long)i * P.d_stride + P.frame0 + t, 1.0f / (float)N);
 
         // ---- pass 2: this thread's k1 = w*KPT + e; X[k1 + R1 k2] = FFT_R2 over r
 #pragma unroll
@@ -249,6 +252,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) {
                         float2 v = y[bitrev(k2, ilog2(R2))];
+                        if (DELAY) v = apply_delay_gain(v, gn, k1 + ((k2 < R2 / 2) ? R1 * k2 : R1 * k2 - N));
                         const int pk = (k2 < R2 / 2) ? (N / 2 + R1 * k2) : (R1 * k2 - N / 2);   // p - k1
                         if (SCALE) {
                             const float f = __ldg(swp + pk);
@@ -268,6 +272,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
                     const int p = u + half;                                  // centre order
                     if (p < 0 || p >= P.K) continue;                         // keep the central K channels (L611)
                     float2 v = y[bitrev(k2, ilog2(R2))];
+                    if (DELAY) v = apply_delay_gain(v, gn, u);
                     if (SCALE) {
                         const float f = __ldg(&P.sw[p]);                     // sqrt(w_p): shared edge / DC exclusion
                         v.x *= f;

@@ -129,37 +129,39 @@ int upload(T **dptr, const std::vector<T> &h)
 
 // power-of-two register kernel: (N, R1, PTS) per supported length; FULL = every bin kept, SCALE = sw[] applied
 template <int N, int R1, int PTS>
-int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, int groups, int chunks, cudaStream_t st)
+int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, bool delay, int groups, int chunks, cudaStream_t st)
 {
     using C = mwax::FPow2Config<N, R1, PTS>;
     static bool attr_set = false;
     if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<N, R1, PTS, true, false>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<N, R1, PTS, true, true>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e == cudaSuccess)
-            e = cudaFuncSetAttribute(mwax::f_stage_pow2_kernel<N, R1, PTS, false, true>,
-                                     cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
-        if (e != cudaSuccess) return MWAX_ERR_CUDA;
+        const void *kerns[5] = {(const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, true, false, false>,
+                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, false>,
+                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, false>,
+                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, true>,
+                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, true>};
+        for (const void *k : kerns)
+            if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
+                return MWAX_ERR_CUDA;
         attr_set = true;
     }
     dim3 grid(groups, chunks);
-    if (full && !scale)
-        mwax::f_stage_pow2_kernel<N, R1, PTS, true, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+    if (delay) {   // the delay variants always take the (all-ones when unused) weight table
+        if (full) mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+        else mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+    } else if (full && !scale)
+        mwax::f_stage_pow2_kernel<N, R1, PTS, true, false, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
     else if (full)
-        mwax::f_stage_pow2_kernel<N, R1, PTS, true, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+        mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
     else
-        mwax::f_stage_pow2_kernel<N, R1, PTS, false, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+        mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, false><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
     return MWAX_OK;
 }
 
-template <bool FULL, bool SCALE, int Q>
+template <bool FULL, bool SCALE, int Q, bool DELAY = false>
 int launch_f_6400p3_q(const mwax::FParams &fp, cudaStream_t st)
 {
     using C = mwax::F6400P3;
-    auto kern = mwax::f_stage_6400p3_kernel<FULL, SCALE, Q>;
+    auto kern = mwax::f_stage_6400p3_kernel<FULL, SCALE, Q, DELAY>;
     static int max_clusters = 0;
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute attr[1];
@@ -183,8 +185,12 @@ int launch_f_6400p3_q(const mwax::FParams &fp, cudaStream_t st)
 }
 
 template <int Q>
-int launch_f_6400p3(const mwax::FParams &fp, bool full, bool scale, cudaStream_t st)
+int launch_f_6400p3(const mwax::FParams &fp, bool full, bool scale, bool delay, cudaStream_t st)
 {
+    if (delay) {   // delay variants exist for the default cluster size only and always take the weight codes
+        if (full) return launch_f_6400p3_q<true, true, 2, true>(fp, st);
+        return launch_f_6400p3_q<false, true, 2, true>(fp, st);
+    }
     if (full && !scale) return launch_f_6400p3_q<true, false, Q>(fp, st);
     if (full) return launch_f_6400p3_q<true, true, Q>(fp, st);
     return launch_f_6400p3_q<false, true, Q>(fp, st);
@@ -270,6 +276,8 @@ struct mwax_corr {
     size_t in_bytes;
     float *d_out;
     size_t out_bytes;
+    const float *d_delay, *d_phase;        // caller-owned delay / phase tables (mwax_corr_set_delays), NULL = off
+    size_t d_row_stride, d_coarse_stride;
     cudaStream_t s_in, s_out;              // copy streams of process_host
     cudaEvent_t ev_start, ev_copied;
     std::vector<cudaEvent_t> ev_in, ev_done;
@@ -461,7 +469,7 @@ int mwax_corr_set_option(mwax_corr_t *h, int key, int value)
     return MWAX_ERR_INVALID_ARG;
 }
 
-int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, void *stream)
+static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, int frame0, int coarse, void *stream)
 {
     if (!h || !d_volt) return MWAX_ERR_NULL;
     if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
@@ -473,12 +481,16 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
     fp.vec_ok = (h->N % 8 == 0) && (row_pitch % 8 == 0) && ((reinterpret_cast<uintptr_t>(d_volt) & 15u) == 0);
     fp.tw = h->d_tw; fp.swcode = h->d_swcode; fp.sw = h->d_sw; fp.in_scale = h->in_scale; fp.chan_scale = h->chan_scale;
     fp.Y = reinterpret_cast<__half2 *>(h->d_Y); fp.pitch2 = h->pitch / 2;
+    const bool delay = h->d_delay || h->d_phase;
+    fp.delay = h->d_delay ? h->d_delay + (size_t)coarse * h->d_coarse_stride : nullptr;
+    fp.phase = h->d_phase ? h->d_phase + (size_t)coarse * h->d_coarse_stride : nullptr;
+    fp.d_stride = (long long)h->d_row_stride; fp.frame0 = frame0;
     fp.y_p_stride = (unsigned)h->T * (unsigned)(h->pitch / 2); fp.y_t_stride = (unsigned)(h->pitch / 2);
     cudaStream_t st = (cudaStream_t)stream;
     if (h->f_kind == 6400) {
         const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
-        int rc = h->f_p3 == 8 ? launch_f_6400p3<8>(fp, full, scale, st) : h->f_p3 == 4 ? launch_f_6400p3<4>(fp, full, scale, st)
-                                                                        : launch_f_6400p3<2>(fp, full, scale, st);
+        int rc = h->f_p3 == 8 ? launch_f_6400p3<8>(fp, full, scale, delay, st) : h->f_p3 == 4 ? launch_f_6400p3<4>(fp, full, scale, delay, st)
+                                                                        : launch_f_6400p3<2>(fp, full, scale, delay, st);
         if (rc != MWAX_OK) return rc;
     } else if (h->f_kind) {
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
@@ -491,10 +503,10 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
         const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
         int rc;
         switch (h->f_kind) {
-            case 64: rc = launch_f_pow2<64, 8, 16>(fp, full, scale, groups, chunks, st); break;
-            case 128: rc = launch_f_pow2<128, 8, 16>(fp, full, scale, groups, chunks, st); break;
-            case 256: rc = launch_f_pow2<256, 16, 32>(fp, full, scale, groups, chunks, st); break;
-            default: rc = launch_f_pow2<512, 16, 32>(fp, full, scale, groups, chunks, st); break;
+            case 64: rc = launch_f_pow2<64, 8, 16>(fp, full, scale, delay, groups, chunks, st); break;
+            case 128: rc = launch_f_pow2<128, 8, 16>(fp, full, scale, delay, groups, chunks, st); break;
+            case 256: rc = launch_f_pow2<256, 16, 32>(fp, full, scale, delay, groups, chunks, st); break;
+            default: rc = launch_f_pow2<512, 16, 32>(fp, full, scale, delay, groups, chunks, st); break;
         }
         if (rc != MWAX_OK) return rc;
     } else {
@@ -502,6 +514,19 @@ int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, vo
         mwax::f_stage_generic_kernel<<<grid, 256, h->f_smem, st>>>(fp);
     }
     return note_cuda(&h->last_cuda);
+}
+
+int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, void *stream)
+{
+    return f_stage_impl(h, d_volt, row_pitch, 0, 0, stream);
+}
+
+int mwax_corr_set_delays(mwax_corr_t *h, const float *d_delay, const float *d_phase, size_t row_stride, size_t coarse_stride)
+{
+    if (!h) return MWAX_ERR_NULL;
+    if ((d_delay || d_phase) && row_stride < (size_t)h->T) return MWAX_ERR_INVALID_ARG;
+    h->d_delay = d_delay; h->d_phase = d_phase; h->d_row_stride = row_stride; h->d_coarse_stride = coarse_stride;
+    return MWAX_OK;
 }
 
 int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
@@ -533,7 +558,8 @@ int mwax_corr_process_batch(mwax_corr_t *h, const int8_t *d_volt, size_t row_pit
     const size_t vis_floats = (size_t)h->C * ((size_t)h->n * (h->n + 1) / 2) * 2;
     for (int c = 0; c < n_coarse; ++c)
         for (int d = 0; d < n_dumps; ++d) {
-            int rc = mwax_corr_f_stage(h, d_volt + 2 * (c * coarse_pitch + d * dump_samples), row_pitch, stream);
+            if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)(d + 1) * h->T) return MWAX_ERR_INVALID_ARG;
+            int rc = f_stage_impl(h, d_volt + 2 * (c * coarse_pitch + d * dump_samples), row_pitch, d * h->T, c, stream);
             if (rc != MWAX_OK) return rc;
             rc = mwax_corr_x_stage(h, d_vis + ((size_t)c * n_dumps + d) * vis_floats, stream);
             if (rc != MWAX_OK) return rc;
@@ -603,7 +629,8 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
             cudaEventRecord(h->ev_in[e], h->s_in);
             cudaStreamWaitEvent(st, h->ev_in[e], 0);
             if (c > 0) cudaStreamWaitEvent(st, h->ev_copied, 0);   // previous channel's visibilities have left d_out
-            int rc = mwax_corr_f_stage(h, h->d_in + 2 * d * dump_samples, row_samples, st);
+            if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)(d + 1) * h->T) return MWAX_ERR_INVALID_ARG;
+            int rc = f_stage_impl(h, h->d_in + 2 * d * dump_samples, row_samples, d * h->T, c, st);
             if (rc != MWAX_OK) return rc;
             rc = mwax_corr_x_stage(h, h->d_out + (size_t)d * vis_floats, st);
             if (rc != MWAX_OK) return rc;

@@ -267,3 +267,68 @@ def test_host_buffer_entry_matches_device_entry():
     torch.cuda.synchronize()
     assert torch.equal(hout, dev.cpu())
     h.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# fractional-delay / phase correction fused into the F kernels (PAPER.md 2.5.1 L266-272)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,N,K,T,F", [
+    (16, 64, 64, 12, 1),        # register kernel, every bin kept
+    (20, 128, 96, 9, 4),        # register kernel, keep < fft, averaging weights
+    (33, 256, 256, 5, 2),       # ragged input group, shared edge taps
+    (12, 100, 100, 7, 5),       # generic Stockham kernel
+    (10, 6400, 6400, 3, 50),    # the paper's mode: three-pass cluster kernel, ragged group
+    (6, 6400, 5000, 2, 50),     # keep < fft at N = 6400
+])
+def test_delay_phase_correction_elementwise(n, N, K, T, F):
+    rng = np.random.default_rng(100 + n + N)
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.3, tones=[synth.Tone(min(3, K // 2 - 1), 6.0, 1)], seed=2000 + n + N)
+    volt = synth.gauss_voltages(spec)
+    delay = rng.uniform(-0.5, 0.5, size=(n, T)).astype(np.float32)       # a different value every frame (fringe stopping)
+    phase = rng.uniform(-np.pi, np.pi, size=(n, T)).astype(np.float32)
+    ref = oracle.fx(volt, N, K, T, F, delay=delay.astype(np.float64), phase=phase.astype(np.float64))
+    plain = oracle.fx(volt, N, K, T, F)
+    h = corr.MwaxCorr(n, N, K, T, F)
+    v = torch.from_numpy(volt).cuda()
+    out = h.new_output()
+    h.set_delays(torch.from_numpy(delay).cuda(), torch.from_numpy(phase).cuda())
+    h.process(v, out[0, 0])
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy()[0, 0])
+    assert _norm_err(got, ref, n) <= TOL
+    assert _norm_err(got, plain, n) > 0.05, "the correction must change the cross products"
+    # delay only / phase only / off again
+    h.set_delays(torch.from_numpy(delay).cuda(), None)
+    h.process(v, out[0, 0])
+    torch.cuda.synchronize()
+    assert _norm_err(_complex(out.cpu().numpy()[0, 0]), oracle.fx(volt, N, K, T, F, delay=delay.astype(np.float64)), n) <= TOL
+    h.set_delays(None, None)
+    h.process(v, out[0, 0])
+    torch.cuda.synchronize()
+    assert _norm_err(_complex(out.cpu().numpy()[0, 0]), plain, n) <= TOL
+    h.destroy()
+
+
+def test_delay_tables_follow_dumps_and_coarse_channels():
+    n, N, T, D, NC = 8, 64, 6, 2, 2
+    rng = np.random.default_rng(3)
+    volt = np.stack([synth.gauss_voltages(synth.GaussSpec(n, N * T * D, N, sigma=16.0, rho=0.2, tones=[], seed=31, coarse=c))
+                     for c in range(NC)])
+    delay = rng.uniform(-0.5, 0.5, size=(NC, n, T * D)).astype(np.float32)
+    phase = rng.uniform(-3, 3, size=(NC, n, T * D)).astype(np.float32)
+    h = corr.MwaxCorr(n, N, N, T, 1)
+    out = h.new_output(n_dumps=D, n_coarse=NC)
+    h.set_delays(torch.from_numpy(delay).cuda(), torch.from_numpy(phase).cuda())
+    h.process_batch(torch.from_numpy(volt).cuda(), out, D, NC)
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy())
+    for c in range(NC):
+        for d in range(D):
+            ref = oracle.fx(volt[c], N, N, T, 1, dump=d, delay=delay[c].astype(np.float64), phase=phase[c].astype(np.float64))
+            assert _norm_err(got[c, d], ref, n) <= TOL
+    # a table shorter than the frames of the batch is refused
+    short = torch.zeros((n, T), dtype=torch.float32, device="cuda")
+    h.set_delays(short, None)
+    with pytest.raises(corr.MwaxError):
+        h.process_batch(torch.from_numpy(volt).cuda(), out, D, NC)
+    h.destroy()
