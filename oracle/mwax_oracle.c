@@ -321,6 +321,38 @@ int mwax_oracle_fx(int n_sel, const int *sel, int N, int K, int T, int F, int mo
     return mwax_oracle_fx_delay(n_sel, sel, N, K, T, F, mode, dump, volt, row_pitch, NULL, NULL, 0, vis_ri);
 }
 
+/* Step 7 (PAPER.md 2.7 L318-326, Fig. 8, Fig. 9): MWAX_ORDER,
+ * "(slowest-to-fastest changing): [time][baseline][channel][polarisation]", baselines listed as antA <= antB row by
+ * row (0-0, 0-1, ..., 0-(n-1), 1-1, ...), polarisation products xx, xy, yx, yy, each value complex.
+ * Readings: Q20 signal path i = 2*tile + pol with pol x = 0, y = 1 (the xGPU input order
+ * "[tile][polarisation]", L274); Q21 element (antA, antB, ch, pq) = sum X_{antA,p} * conj(X_{antB,q}) -- the
+ * first-named antenna unconjugated, as in step 4 (Q2; which antenna the instrument conjugates is unpinned).
+ * With the native packed triangle V[ch][i(i+1)/2 + j] (i >= j) that is V[i][j] when i >= j, else conj(V[j][i]).
+ * in:  V  [C][n(n+1)/2] complex double, n = 2*n_tiles signal paths.
+ * out: M  [n_tiles(n_tiles+1)/2][C][4] complex double;  W [n_tiles(n_tiles+1)/2][4] weights, all 1.0 (L328: "these
+ * weights are not utilised and all values are set to 1.0"). */
+int mwax_oracle_mwax_order(int n_tiles, int C, const double *V_ri, double *M_ri, double *W)
+{
+    if (n_tiles < 1 || C < 1 || !V_ri || !M_ri) return ORACLE_ERR_ARG;
+    const cplx *V = (const cplx *)V_ri;
+    cplx *M = (cplx *)M_ri;
+    const size_t n = 2 * (size_t)n_tiles, B = n * (n + 1) / 2;
+    size_t row = 0;
+    for (int a = 0; a < n_tiles; ++a)
+        for (int b = a; b < n_tiles; ++b, ++row)
+            for (int ch = 0; ch < C; ++ch)
+                for (int p = 0; p < 2; ++p)
+                    for (int q = 0; q < 2; ++q) {
+                        const size_t i = 2 * (size_t)a + p, j = 2 * (size_t)b + q;
+                        const cplx v = (i >= j) ? V[(size_t)ch * B + i * (i + 1) / 2 + j]
+                                                : conj(V[(size_t)ch * B + j * (j + 1) / 2 + i]);
+                        M[(row * C + ch) * 4 + 2 * p + q] = v;
+                    }
+    if (W)
+        for (size_t r = 0; r < row * 4; ++r) W[r] = 1.0;
+    return ORACLE_OK;
+}
+
 /* Integer X-only path (BASELINE.json configs[1]; the same contraction as step 4 on pre-channelised int8
  * samples z = a + ib, layout [chan][time][input][re,im]):
  *   Re V_ab = sum_t (a_a a_b + b_a b_b),  Im V_ab = sum_t (b_a a_b - a_a b_b)      (z_a * conj(z_b))

@@ -51,6 +51,7 @@ def _load():
                                                  dp, dp, ctypes.c_int64, dp]
         lib.mwax_oracle_fx_delay.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                              ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp, dp, ctypes.c_int64, dp]
+        lib.mwax_oracle_mwax_order.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp, dp]
         lib.mwax_oracle_xcorr_i8.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, i8p, i32p]
         lib.mwax_oracle_threads.argtypes = []
         _lib = lib
@@ -167,6 +168,18 @@ def fx(volt: np.ndarray, N: int, K: int, T: int, F: int, mode: int = AVG_CENTRE_
                                         volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), volt.shape[1],
                                         dpp, php, stride, _dp(V.view(np.float64))), "fx")
     return V
+
+
+def mwax_order(V: np.ndarray, n_inputs: int):
+    """Step 7: native V complex128 [C][n(n+1)/2] -> (M complex128 [n_tiles(n_tiles+1)/2][C][4], W float64 [..][4])."""
+    V = np.ascontiguousarray(V, dtype=np.complex128)
+    C, B = V.shape
+    assert n_inputs % 2 == 0 and B == n_inputs * (n_inputs + 1) // 2
+    nt = n_inputs // 2
+    M = np.empty((nt * (nt + 1) // 2, C, 4), dtype=np.complex128)
+    W = np.empty((nt * (nt + 1) // 2, 4), dtype=np.float64)
+    _check(_load().mwax_oracle_mwax_order(nt, C, _dp(V.view(np.float64)), _dp(M.view(np.float64)), _dp(W)), "mwax_order")
+    return M, W
 
 
 def xcorr_i8(z: np.ndarray, sel=None) -> np.ndarray:

@@ -425,3 +425,39 @@ def test_fractional_delay_flattens_the_phase_of_a_delayed_copy():
     Vc = oracle.fx(volt, N, N, T, 1, delay=np.array([[0.0] * T, [-tau] * T]))[:, b]
     assert np.abs(np.angle(Vc[sel])).max() < 0.05            # corrected: flat
     assert np.abs(np.angle(V[sel])).max() > 0.5
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Step 7: MWAX_ORDER (PAPER.md 2.7 L318-326, Figs 8-9)
+# ------------------------------------------------------------------------------------------------------------------
+def test_mwax_order_fig8_rows_and_bruteforce_products():
+    """Fig. 8's example: 4 tiles, 2 channels -> 10 baseline rows in the printed order, channel faster than baseline,
+    xx xy yx yy fastest; every element equals the product sum formed directly from the spectra with numpy."""
+    n_tiles, want_rows = [int(x) for x in np.loadtxt(os.path.join(GOLDEN, "fig8_baseline_rows.txt"), dtype=int)]
+    assert (n_tiles, want_rows) == (4, 10)
+    n, N, K, T = 2 * n_tiles, 8, 2, 5
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.4, tones=[], seed=808)
+    volt = synth.gauss_voltages(spec)
+    Y = oracle.spectra(volt, N, K, T)                      # [K][T][n]
+    V = oracle.average(oracle.correlate(Y), n, 1)
+    M, W = oracle.mwax_order(V, n)
+    assert M.shape == (want_rows, K, 4) and W.shape == (want_rows, 4) and np.all(W == 1.0)
+    rows = [(a, b) for a in range(n_tiles) for b in range(a, n_tiles)]
+    assert rows == [(0, 0), (0, 1), (0, 2), (0, 3), (1, 1), (1, 2), (1, 3), (2, 2), (2, 3), (3, 3)]   # as printed in Fig. 8
+    for r, (a, b) in enumerate(rows):
+        for ch in range(K):
+            for p in range(2):
+                for q in range(2):
+                    direct = np.sum(Y[ch, :, 2 * a + p] * np.conj(Y[ch, :, 2 * b + q]))
+                    assert abs(M[r, ch, 2 * p + q] - direct) <= 1e-9 * max(1.0, abs(direct))
+    # autos: xx and yy real, xy = conj(yx)
+    for r, (a, b) in enumerate(rows):
+        if a == b:
+            assert np.all(M[r, :, 0].imag == 0) and np.all(M[r, :, 3].imag == 0)
+            assert np.allclose(M[r, :, 1], np.conj(M[r, :, 2]))
+
+
+def test_mwax_order_value_count_matches_the_paper():
+    """128 tiles: 8256 baselines x 4 polarisation products = 33 024 values per channel (Fig. 8's format; DESIGN Q16)."""
+    nt = 128
+    assert nt * (nt + 1) // 2 * 4 == 33024
