@@ -284,6 +284,19 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
     res["f_ms_delay"] = d0.elapsed_time(d1) / n_rep
     h.set_delays(None, None)
 
+    # ---- MWAX_ORDER emitter on one dump (PAPER.md 2.7: 0.6-1.8 s of CPU time per 8 s in Table 2)
+    mo = h.to_mwax_order(vis[0, 0])
+    o0 = torch.cuda.Event(enable_timing=True)
+    o1 = torch.cuda.Event(enable_timing=True)
+    o0.record(stream)
+    for _ in range(n_rep):
+        h.to_mwax_order(vis[0, 0], mo)
+    o1.record(stream)
+    torch.cuda.synchronize()
+    res["order_ms"] = o0.elapsed_time(o1) / n_rep
+    res["order_gbs"] = (vis[0, 0].numel() * 4 + mo.numel() * 4) / (res["order_ms"] * 1e-3) / 1e9
+    del mo
+
     # ---- e2e through the public host-buffer call (H2D + D2H inside the timed region)
     if do_e2e:
         hvis = torch.empty((1, D, C, B, 2), dtype=torch.float32).pin_memory()
@@ -389,6 +402,8 @@ def main():
                 "clocks": res["clocks"],
                 "roofline": roof_x if x_dom else roof_f,
                 "stages": {"f": roof_f, "x": roof_x},
+                "next_rows": {"mwax_order_ms_per_dump": res.get("order_ms"), "mwax_order_gbs": res.get("order_gbs"),
+                              "f_stage_ms_with_delay_phase_correction": res.get("f_ms_delay")},
                 "paper_context": "MWAX on 1 x A40 + 2 x Epyc 7F72: 5.9 s per 8 s subfile at 256 tiles, 1 s/10 kHz mode "
                                  "=> 1 coarse channel per GPU in real time (PAPER.md Table 2 L531-545)"}
         if other is not None:

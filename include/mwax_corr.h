@@ -115,6 +115,18 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
 int mwax_corr_f_stage(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, void *stream);
 int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream);
 
+/* MWAX_ORDER emitter (§2.7, Figs 8-9): re-index one dump from the native
+ * packed triangle into the instrument's output order, on the device.
+ *   d_vis      in : float [C][n(n+1)/2][re,im], as written by process() (n_inputs must be even: signal path
+ *                   i = 2*tile + pol, pol x = 0, y = 1, reading Q20)
+ *   d_out      out: float [n_tiles(n_tiles+1)/2][C][xx,xy,yx,yy][re,im], baselines antA <= antB row by row
+ *                   (0-0, 0-1, ..., 0-(nt-1), 1-1, ...); element (antA, antB, ch, pq) = sum X_{antA,p} conj(X_{antB,q})
+ *                   (reading Q21).  mwax_corr_mwax_order_bytes() bytes.
+ *   d_weights  out: float [n_tiles(n_tiles+1)/2][4] visibility weights, all 1.0 (L328), or NULL
+ * Pure data movement: the values are bit copies (sign of Im flipped where the conjugate is taken). */
+int mwax_corr_to_mwax_order(mwax_corr_t *h, const float *d_vis, float *d_out, float *d_weights, void *stream);
+size_t mwax_corr_mwax_order_bytes(const mwax_corr_t *h);
+
 size_t mwax_corr_input_bytes(const mwax_corr_t *h);
 size_t mwax_corr_output_bytes(const mwax_corr_t *h);
 size_t mwax_corr_workspace_bytes(const mwax_corr_t *h);

@@ -15,7 +15,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libmwax_corr.so")
-_SOURCES = ["mwax_api.cu", "f_stage.cuh", "f_stage_pow2.cuh", "f_stage_6400p3.cuh", "x_stage.cuh", "x_stage2.cuh", "ptx.cuh"]
+_SOURCES = ["mwax_api.cu", "mwax_order.cuh", "f_stage.cuh", "f_stage_pow2.cuh", "f_stage_6400p3.cuh", "x_stage.cuh", "x_stage2.cuh", "ptx.cuh"]
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "mwax_corr.h")
 _lib = None
 
@@ -72,6 +72,9 @@ def lib() -> ctypes.CDLL:
         L.mwax_corr_process_host.argtypes = [vp, vp, sz, sz, i32, i32, vp, vp]
         L.mwax_corr_f_stage.argtypes = [vp, vp, sz, vp]
         L.mwax_corr_set_delays.argtypes = [vp, vp, vp, sz, sz]
+        L.mwax_corr_to_mwax_order.argtypes = [vp, vp, vp, vp, vp]
+        L.mwax_corr_mwax_order_bytes.restype = sz
+        L.mwax_corr_mwax_order_bytes.argtypes = [vp]
         L.mwax_corr_x_stage.argtypes = [vp, vp, vp]
         for f in ("input_bytes", "output_bytes", "workspace_bytes"):
             getattr(L, "mwax_corr_" + f).restype = sz
@@ -185,6 +188,22 @@ class MwaxCorr:
         _check(lib().mwax_corr_set_delays(self._h, delay.data_ptr() if delay is not None else None,
                                           phase.data_ptr() if phase is not None else None, row_stride,
                                           row_stride * self.n_inputs), "mwax_corr_set_delays", self._h)
+
+    def to_mwax_order(self, vis: torch.Tensor, out: torch.Tensor | None = None, weights: torch.Tensor | None = None,
+                      stream=None):
+        """vis float32 cuda [C][B][2] (one dump) -> out float32 cuda [n_tiles(n_tiles+1)/2][C][4][2] (+ weights [..][4])."""
+        assert vis.is_cuda and vis.dtype == torch.float32 and vis.is_contiguous() and vis.numel() * 4 == self.output_bytes()
+        nt = self.n_inputs // 2
+        if out is None:
+            out = torch.empty((nt * (nt + 1) // 2, self.n_out, 4, 2), dtype=torch.float32, device=vis.device)
+        assert out.is_cuda and out.dtype == torch.float32 and out.is_contiguous()
+        assert out.numel() * 4 == lib().mwax_corr_mwax_order_bytes(self._h)
+        if weights is not None:
+            assert weights.is_cuda and weights.dtype == torch.float32 and weights.numel() == nt * (nt + 1) // 2 * 4
+        _check(lib().mwax_corr_to_mwax_order(self._h, vis.data_ptr(), out.data_ptr(),
+                                             weights.data_ptr() if weights is not None else None, _stream_ptr(stream)),
+               "mwax_corr_to_mwax_order", self._h)
+        return out
 
     def f_stage(self, volt: torch.Tensor, row_pitch: int | None = None, stream=None):
         assert volt.is_cuda and volt.dtype == torch.int8 and volt.is_contiguous()

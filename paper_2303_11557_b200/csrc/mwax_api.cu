@@ -18,6 +18,7 @@
 #include "f_stage_6400p3.cuh"
 #include "x_stage.cuh"
 #include "x_stage2.cuh"
+#include "mwax_order.cuh"
 
 namespace {
 
@@ -653,6 +654,26 @@ size_t mwax_corr_output_bytes(const mwax_corr_t *h)
 {
     return h ? (size_t)h->C * ((size_t)h->n * (h->n + 1) / 2) * 8 : 0;
 }
+size_t mwax_corr_mwax_order_bytes(const mwax_corr_t *h)
+{
+    if (!h || (h->n & 1)) return 0;
+    const size_t nt = (size_t)h->n / 2;
+    return nt * (nt + 1) / 2 * (size_t)h->C * 4 * 8;
+}
+
+int mwax_corr_to_mwax_order(mwax_corr_t *h, const float *d_vis, float *d_out, float *d_weights, void *stream)
+{
+    if (!h || !d_vis || !d_out) return MWAX_ERR_NULL;
+    if (h->n & 1) return MWAX_ERR_UNSUPPORTED;              // tiles are pairs of signal paths (x, y)
+    mwax::OrderParams op;
+    op.vis = reinterpret_cast<const float2 *>(d_vis); op.out = reinterpret_cast<float2 *>(d_out); op.weights = d_weights;
+    op.n_tiles = h->n / 2; op.C = h->C; op.chan_stride = (long long)h->n * (h->n + 1) / 2;
+    dim3 grid((op.n_tiles + mwax::ORD_TA - 1) / mwax::ORD_TA, op.n_tiles, (op.C + mwax::ORD_TC - 1) / mwax::ORD_TC);
+    if (grid.y > 65535 || grid.z > 65535) return MWAX_ERR_UNSUPPORTED;
+    mwax::mwax_order_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(op);
+    return note_cuda(&h->last_cuda);
+}
+
 size_t mwax_corr_workspace_bytes(const mwax_corr_t *h) { return h ? h->y_bytes : 0; }
 int mwax_corr_launches_per_process(const mwax_corr_t *h) { return h ? 2 : 0; }
 int mwax_corr_last_cuda_error(const mwax_corr_t *h) { return h ? h->last_cuda : 0; }

@@ -332,3 +332,52 @@ def test_delay_tables_follow_dumps_and_coarse_channels():
     with pytest.raises(corr.MwaxError):
         h.process_batch(torch.from_numpy(volt).cuda(), out, D, NC)
     h.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# MWAX_ORDER emitter (PAPER.md 2.7 L318-326, Figs 8-9) — index work, bit-exact
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,C", [(8, 2), (70, 5), (34, 25), (512, 128)])
+def test_mwax_order_reindexing_is_bit_exact(n, C):
+    """Host-made native array (not from the CUDA path) -> device re-index vs the oracle's step 7, element for element."""
+    rng = np.random.default_rng(n * 1000 + C)
+    B = n * (n + 1) // 2
+    nat = rng.standard_normal((C, B, 2)).astype(np.float32)
+    ii = np.arange(n)
+    nat[:, ii * (ii + 1) // 2 + ii, 1] = 0.0                 # autos are real
+    h = corr.MwaxCorr(n, C, C, 1, 1)                         # the call only uses (n, C) of the plan
+    assert h.n_out == C
+    nt = n // 2
+    out = torch.full((nt * (nt + 1) // 2, C, 4, 2), float("nan"), dtype=torch.float32, device="cuda")
+    wts = torch.zeros((nt * (nt + 1) // 2, 4), dtype=torch.float32, device="cuda")
+    h.to_mwax_order(torch.from_numpy(nat).cuda(), out, wts)
+    torch.cuda.synchronize()
+    M, W = oracle.mwax_order(nat[..., 0].astype(np.float64) + 1j * nat[..., 1].astype(np.float64), n)
+    got = out.cpu().numpy()
+    assert np.array_equal(got[..., 0], M.real.astype(np.float32)) and np.array_equal(got[..., 1], M.imag.astype(np.float32))
+    assert np.array_equal(wts.cpu().numpy(), W.astype(np.float32))
+    h.destroy()
+
+
+def test_fx_then_mwax_order_matches_oracle():
+    n, N, T = 12, 64, 20
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.3, tones=[synth.Tone(7, 5.0, 1)], seed=4242)
+    volt = synth.gauss_voltages(spec)
+    ref = oracle.fx(volt, N, N, T, 4)
+    Mref, _ = oracle.mwax_order(ref, n)
+    h = corr.MwaxCorr(n, N, N, T, 4)
+    vis = h.new_output()[0, 0]
+    h.process(torch.from_numpy(volt).cuda(), vis)
+    out = h.to_mwax_order(vis)
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy())                        # [rows][C][4]
+    A = np.array([ref[:, oracle.baseline_index(i, i)].real for i in range(n)])      # [n][C]
+    row = 0
+    for a in range(n // 2):
+        for b in range(a, n // 2):
+            for p in range(2):
+                for q in range(2):
+                    norm = np.sqrt(A[2 * a + p] * A[2 * b + q])
+                    assert np.all(np.abs(got[row, :, 2 * p + q] - Mref[row, :, 2 * p + q]) <= TOL * norm)
+            row += 1
+    h.destroy()
