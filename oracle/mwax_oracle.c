@@ -353,6 +353,33 @@ int mwax_oracle_mwax_order(int n_tiles, int C, const double *V_ri, double *M_ri,
     return ORACLE_OK;
 }
 
+/* Step 8 (PAPER.md 4.1 L557-559, 2.4.2 L225, 2.6 L288): visibility weights = "the fraction of
+ * the integration time for that visibility set that contained fully populated 50 ms sub-blocks in both signal paths
+ * for that baseline/polarisation", from the zeroing flags (1 = that sub-block of that signal path was zeroed), and the
+ * optional normalisation "such that missing packets do not cause variations in visibility magnitudes".
+ * Reading Q22: weight(antA, antB, pq) = (1/S) * #{s : both paths valid in sub-block s}; normalising divides the
+ * visibility by its weight; a weight of 0 leaves the (necessarily zero) visibility untouched.
+ * flags: [2*n_tiles][S] bytes.  W: [n_tiles(n_tiles+1)/2][4].  M (optional, normalised in place): [rows][C][4] complex. */
+int mwax_oracle_occupancy(int n_tiles, int S, const uint8_t *flags, int C, int normalise, double *W, double *M_ri)
+{
+    if (n_tiles < 1 || S < 1 || !flags || !W) return ORACLE_ERR_ARG;
+    cplx *M = (cplx *)M_ri;
+    size_t row = 0;
+    for (int a = 0; a < n_tiles; ++a)
+        for (int b = a; b < n_tiles; ++b, ++row)
+            for (int p = 0; p < 2; ++p)
+                for (int q = 0; q < 2; ++q) {
+                    const uint8_t *fa = flags + (size_t)(2 * a + p) * S, *fb = flags + (size_t)(2 * b + q) * S;
+                    int both = 0;
+                    for (int sb = 0; sb < S; ++sb) both += (!fa[sb] && !fb[sb]);
+                    const double w = (double)both / (double)S;
+                    W[row * 4 + 2 * p + q] = w;
+                    if (normalise && M && w > 0.0)
+                        for (int ch = 0; ch < C; ++ch) M[(row * C + ch) * 4 + 2 * p + q] /= w;
+                }
+    return ORACLE_OK;
+}
+
 /* Integer X-only path (BASELINE.json configs[1]; the same contraction as step 4 on pre-channelised int8
  * samples z = a + ib, layout [chan][time][input][re,im]):
  *   Re V_ab = sum_t (a_a a_b + b_a b_b),  Im V_ab = sum_t (b_a a_b - a_a b_b)      (z_a * conj(z_b))

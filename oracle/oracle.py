@@ -52,6 +52,8 @@ def _load():
         lib.mwax_oracle_fx_delay.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                              ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp, dp, ctypes.c_int64, dp]
         lib.mwax_oracle_mwax_order.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp, dp]
+        lib.mwax_oracle_occupancy.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_uint8), ctypes.c_int,
+                                              ctypes.c_int, dp, dp]
         lib.mwax_oracle_xcorr_i8.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, i8p, i32p]
         lib.mwax_oracle_threads.argtypes = []
         _lib = lib
@@ -180,6 +182,24 @@ def mwax_order(V: np.ndarray, n_inputs: int):
     W = np.empty((nt * (nt + 1) // 2, 4), dtype=np.float64)
     _check(_load().mwax_oracle_mwax_order(nt, C, _dp(V.view(np.float64)), _dp(M.view(np.float64)), _dp(W)), "mwax_order")
     return M, W
+
+
+def occupancy(flags: np.ndarray, M: np.ndarray | None = None, normalise: bool = False):
+    """Step 8: zeroing flags uint8 [n][S] (1 = zeroed) -> weights float64 [n_tiles(n_tiles+1)/2][4]; with M (MWAX_ORDER,
+    complex128 [rows][C][4]) and normalise=True also returns M divided by its weights."""
+    flags = np.ascontiguousarray(flags, dtype=np.uint8)
+    n, S = flags.shape
+    assert n % 2 == 0
+    nt = n // 2
+    W = np.empty((nt * (nt + 1) // 2, 4), dtype=np.float64)
+    Mo, C, mp = None, 0, None
+    if M is not None:
+        Mo = np.array(M, dtype=np.complex128, order="C")
+        C = Mo.shape[1]
+        mp = _dp(Mo.view(np.float64))
+    _check(_load().mwax_oracle_occupancy(nt, S, flags.ctypes.data_as(ctypes.POINTER(ctypes.c_uint8)), C,
+                                         1 if normalise else 0, _dp(W), mp), "occupancy")
+    return (W, Mo) if M is not None else W
 
 
 def xcorr_i8(z: np.ndarray, sel=None) -> np.ndarray:

@@ -461,3 +461,50 @@ def test_mwax_order_value_count_matches_the_paper():
     """128 tiles: 8256 baselines x 4 polarisation products = 33 024 values per channel (Fig. 8's format; DESIGN Q16)."""
     nt = 128
     assert nt * (nt + 1) // 2 * 4 == 33024
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# Step 8: occupancy weights from the zeroing flags (SURVEY.md 8(f) NEXT #3; PAPER.md 4.1 L557-559)
+# ------------------------------------------------------------------------------------------------------------------
+def test_occupancy_weights_bruteforce_and_special_cases():
+    rng = np.random.default_rng(12)
+    nt, S = 5, 16
+    flags = (rng.random((2 * nt, S)) < 0.3).astype(np.uint8)
+    flags[4, :] = 1                                          # a signal path zeroed for the whole integration
+    flags[7, :] = 0                                          # a signal path that lost nothing
+    W = oracle.occupancy(flags)
+    valid = 1 - flags.astype(np.int64)
+    row = 0
+    for a in range(nt):
+        for b in range(a, nt):
+            for p in range(2):
+                for q in range(2):
+                    want = np.mean(valid[2 * a + p] & valid[2 * b + q])      # numpy, nothing of the oracle's loop
+                    assert W[row, 2 * p + q] == want
+            row += 1
+    assert np.all((W >= 0) & (W <= 1))
+    assert np.all(oracle.occupancy(np.zeros((2 * nt, S), np.uint8)) == 1.0)          # "all values are set to 1.0" today (L328)
+    rows = {(a, b): r for r, (a, b) in enumerate((a, b) for a in range(nt) for b in range(a, nt))}
+    assert np.all(W[rows[(2, 2)], 0] == 0) and np.all(W[rows[(0, 2)], [0, 2]] == 0)  # everything with path 4 = (tile 2, x)
+    assert W[rows[(3, 3)], 3] == 1.0                                                # path 7 with itself
+
+
+def test_occupancy_normalisation_restores_visibility_magnitudes():
+    """Zero a quarter of the integration on one signal path: its cross products drop to ~75 %; dividing by the weight
+    brings them back (L559: 'such that missing packets do not cause variations in visibility magnitudes')."""
+    n, N, T, S = 4, 32, 400, 8
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.6, tones=[], seed=99)
+    volt = synth.gauss_voltages(spec)
+    full, _ = oracle.mwax_order(oracle.fx(volt, N, N, T, N), n)       # one output channel (all fine channels averaged)
+    flags = np.zeros((n, S), np.uint8)
+    flags[1, :2] = 1                                                   # path 1 = (tile 0, y): first quarter zeroed
+    vz = volt.copy()
+    vz[1, : N * T // 4] = 0
+    M, _ = oracle.mwax_order(oracle.fx(vz, N, N, T, N), n)
+    W, Mn = oracle.occupancy(flags, M, normalise=True)
+    r01 = 1                                                            # row (antA 0, antB 1)
+    assert W[r01, 2] == 0.75 and W[r01, 0] == 1.0                      # yx involves path 1, xx does not
+    ratio_raw = abs(M[r01, 0, 2]) / abs(full[r01, 0, 2])
+    ratio_norm = abs(Mn[r01, 0, 2]) / abs(full[r01, 0, 2])
+    assert abs(ratio_raw - 0.75) < 0.05 and abs(ratio_norm - 1.0) < 0.05
+    assert np.array_equal(Mn[r01, :, 0], M[r01, :, 0])                 # weight 1.0: untouched
