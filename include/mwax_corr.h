@@ -127,6 +127,14 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream);
 int mwax_corr_to_mwax_order(mwax_corr_t *h, const float *d_vis, float *d_out, float *d_weights, void *stream);
 size_t mwax_corr_mwax_order_bytes(const mwax_corr_t *h);
 
+/* Same with occupancy weights (§4.1, §2.4.2):
+ *   d_flags    in : uint8 [n_inputs][n_sub] zeroing flags of this integration, 1 = that sub-block (50 ms in the paper)
+ *                   of that signal path was zero-filled; NULL = nothing was (weights 1.0)
+ *   normalise     : non-zero divides every visibility by its weight (weight 0 leaves the zero visibility as it is)
+ *   d_weights  out: weight(antA, antB, pq) = fraction of the n_sub sub-blocks in which BOTH signal paths were valid */
+int mwax_corr_to_mwax_order_weighted(mwax_corr_t *h, const float *d_vis, const uint8_t *d_flags, int n_sub, int normalise,
+                                     float *d_out, float *d_weights, void *stream);
+
 size_t mwax_corr_input_bytes(const mwax_corr_t *h);
 size_t mwax_corr_output_bytes(const mwax_corr_t *h);
 size_t mwax_corr_workspace_bytes(const mwax_corr_t *h);

@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.mwax_corr_f_stage.argtypes = [vp, vp, sz, vp]
         L.mwax_corr_set_delays.argtypes = [vp, vp, vp, sz, sz]
         L.mwax_corr_to_mwax_order.argtypes = [vp, vp, vp, vp, vp]
+        L.mwax_corr_to_mwax_order_weighted.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
         L.mwax_corr_mwax_order_bytes.restype = sz
         L.mwax_corr_mwax_order_bytes.argtypes = [vp]
         L.mwax_corr_x_stage.argtypes = [vp, vp, vp]
@@ -190,7 +191,7 @@ class MwaxCorr:
                                           row_stride * self.n_inputs), "mwax_corr_set_delays", self._h)
 
     def to_mwax_order(self, vis: torch.Tensor, out: torch.Tensor | None = None, weights: torch.Tensor | None = None,
-                      stream=None):
+                      stream=None, flags: torch.Tensor | None = None, normalise: bool = False):
         """vis float32 cuda [C][B][2] (one dump) -> out float32 cuda [n_tiles(n_tiles+1)/2][C][4][2] (+ weights [..][4])."""
         assert vis.is_cuda and vis.dtype == torch.float32 and vis.is_contiguous() and vis.numel() * 4 == self.output_bytes()
         nt = self.n_inputs // 2
@@ -200,9 +201,14 @@ class MwaxCorr:
         assert out.numel() * 4 == lib().mwax_corr_mwax_order_bytes(self._h)
         if weights is not None:
             assert weights.is_cuda and weights.dtype == torch.float32 and weights.numel() == nt * (nt + 1) // 2 * 4
-        _check(lib().mwax_corr_to_mwax_order(self._h, vis.data_ptr(), out.data_ptr(),
-                                             weights.data_ptr() if weights is not None else None, _stream_ptr(stream)),
-               "mwax_corr_to_mwax_order", self._h)
+        n_sub = 0
+        if flags is not None:
+            assert flags.is_cuda and flags.dtype == torch.uint8 and flags.is_contiguous() and flags.shape[0] == self.n_inputs
+            n_sub = flags.shape[1]
+        _check(lib().mwax_corr_to_mwax_order_weighted(self._h, vis.data_ptr(), flags.data_ptr() if flags is not None else None,
+                                                      n_sub, 1 if normalise else 0, out.data_ptr(),
+                                                      weights.data_ptr() if weights is not None else None,
+                                                      _stream_ptr(stream)), "mwax_corr_to_mwax_order_weighted", self._h)
         return out
 
     def f_stage(self, volt: torch.Tensor, row_pitch: int | None = None, stream=None):

@@ -663,11 +663,19 @@ size_t mwax_corr_mwax_order_bytes(const mwax_corr_t *h)
 
 int mwax_corr_to_mwax_order(mwax_corr_t *h, const float *d_vis, float *d_out, float *d_weights, void *stream)
 {
+    return mwax_corr_to_mwax_order_weighted(h, d_vis, nullptr, 0, 0, d_out, d_weights, stream);
+}
+
+int mwax_corr_to_mwax_order_weighted(mwax_corr_t *h, const float *d_vis, const uint8_t *d_flags, int n_sub, int normalise,
+                                     float *d_out, float *d_weights, void *stream)
+{
     if (!h || !d_vis || !d_out) return MWAX_ERR_NULL;
+    if (d_flags && n_sub < 1) return MWAX_ERR_INVALID_ARG;
     if (h->n & 1) return MWAX_ERR_UNSUPPORTED;              // tiles are pairs of signal paths (x, y)
     mwax::OrderParams op;
     op.vis = reinterpret_cast<const float2 *>(d_vis); op.out = reinterpret_cast<float2 *>(d_out); op.weights = d_weights;
     op.n_tiles = h->n / 2; op.C = h->C; op.chan_stride = (long long)h->n * (h->n + 1) / 2;
+    op.flags = d_flags; op.n_sub = n_sub; op.normalise = (d_flags && normalise) ? 1 : 0;
     dim3 grid((op.n_tiles + mwax::ORD_TA - 1) / mwax::ORD_TA, op.n_tiles, (op.C + mwax::ORD_TC - 1) / mwax::ORD_TC);
     if (grid.y > 65535 || grid.z > 65535) return MWAX_ERR_UNSUPPORTED;
     mwax::mwax_order_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(op);

@@ -19,6 +19,10 @@ struct OrderParams {
     float *weights;        // [n_tiles(n_tiles+1)/2][4] or nullptr
     int n_tiles, C;
     long long chan_stride; // n(n+1)/2
+    // occupancy weights (§4.1): zeroing flags [2 n_tiles][n_sub] bytes, 1 = that sub-block of that
+    // signal path was zeroed; nullptr = everything valid (weights 1.0).  normalise: divide each visibility by its weight.
+    const uint8_t *flags;
+    int n_sub, normalise;
 };
 
 constexpr int ORD_TA = 16, ORD_TC = 16;
@@ -26,6 +30,7 @@ constexpr int ORD_TA = 16, ORD_TC = 16;
 __global__ void __launch_bounds__(256) mwax_order_kernel(const OrderParams P)
 {
     __shared__ float2 tile[ORD_TC][2][2 * ORD_TA + 1];
+    __shared__ float wt[ORD_TA][4];
     const int b = blockIdx.y;                                  // antB
     const int a0 = blockIdx.x * ORD_TA;                        // first antA of the tile
     const int c0 = blockIdx.z * ORD_TC;
@@ -40,6 +45,18 @@ __global__ void __launch_bounds__(256) mwax_order_kernel(const OrderParams P)
         float2 v = make_float2(0.f, 0.f);
         if (cl < nc && col < 2 * na && j <= i) v = P.vis[(long long)(c0 + cl) * P.chan_stride + i * (i + 1) / 2 + j];
         tile[cl][q][col] = v;
+    }
+    // weight(antA, antB, pq) = fraction of sub-blocks in which BOTH signal paths were fully populated
+    for (int e = threadIdx.x; e < na * 4; e += blockDim.x) {
+        float w = 1.0f;
+        if (P.flags) {
+            const uint8_t *fa = P.flags + (size_t)(2 * (a0 + (e >> 2)) + ((e >> 1) & 1)) * P.n_sub;
+            const uint8_t *fb = P.flags + (size_t)(2 * b + (e & 1)) * P.n_sub;
+            int both = 0;
+            for (int sb = 0; sb < P.n_sub; ++sb) both += (!fa[sb] && !fb[sb]);
+            w = (float)both / (float)P.n_sub;
+        }
+        wt[e >> 2][e & 3] = w;
     }
     __syncthreads();
 
@@ -57,6 +74,10 @@ __global__ void __launch_bounds__(256) mwax_order_kernel(const OrderParams P)
         } else {                                               // a == b, (p, q) = (1, 0): V[2a+1][2a] as stored
             v = tile[cl][1][2 * al];
         }
+        if (P.normalise) {
+            const float w = wt[al][pq];
+            if (w > 0.0f) { v.x /= w; v.y /= w; }
+        }
         const long long row = (long long)a * P.n_tiles - (long long)a * (a - 1) / 2 + (b - a);
         P.out[(row * P.C + c0 + cl) * 4 + pq] = v;
     }
@@ -64,7 +85,7 @@ __global__ void __launch_bounds__(256) mwax_order_kernel(const OrderParams P)
         for (int e = threadIdx.x; e < na * 4; e += blockDim.x) {
             const int a = a0 + (e >> 2);
             const long long row = (long long)a * P.n_tiles - (long long)a * (a - 1) / 2 + (b - a);
-            P.weights[row * 4 + (e & 3)] = 1.0f;               // occupancy weights: "all values are set to 1.0" (L328)
+            P.weights[row * 4 + (e & 3)] = wt[e >> 2][e & 3];   // 1.0 without flags: "all values are set to 1.0" (L328)
         }
     }
 }

@@ -381,3 +381,34 @@ def test_fx_then_mwax_order_matches_oracle():
                     assert np.all(np.abs(got[row, :, 2 * p + q] - Mref[row, :, 2 * p + q]) <= TOL * norm)
             row += 1
     h.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# occupancy weights from zeroing flags + optional normalisation (PAPER.md 4.1 L557-559)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,C,S", [(8, 2, 4), (70, 5, 20), (512, 128, 10)])
+def test_occupancy_weights_and_normalisation(n, C, S):
+    rng = np.random.default_rng(n + C + S)
+    B = n * (n + 1) // 2
+    nat = rng.standard_normal((C, B, 2)).astype(np.float32)
+    ii = np.arange(n)
+    nat[:, ii * (ii + 1) // 2 + ii, 1] = 0.0
+    flags = (rng.random((n, S)) < 0.2).astype(np.uint8)
+    flags[3, :] = 1                                          # a path lost for the whole integration: weight 0
+    h = corr.MwaxCorr(n, C, C, 1, 1)
+    nt = n // 2
+    wts = torch.zeros((nt * (nt + 1) // 2, 4), dtype=torch.float32, device="cuda")
+    M, _ = oracle.mwax_order(nat[..., 0].astype(np.float64) + 1j * nat[..., 1].astype(np.float64), n)
+    W, Mn = oracle.occupancy(flags, M, normalise=True)
+    # weights only: values stay bit copies
+    out = h.to_mwax_order(torch.from_numpy(nat).cuda(), weights=wts, flags=torch.from_numpy(flags).cuda(), normalise=False)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    assert np.array_equal(wts.cpu().numpy(), W.astype(np.float32))             # k/S in fp32 == fp32(k/S in fp64)
+    assert np.array_equal(got[..., 0], M.real.astype(np.float32)) and np.array_equal(got[..., 1], M.imag.astype(np.float32))
+    # normalised: one fp32 division per component
+    out = h.to_mwax_order(torch.from_numpy(nat).cuda(), weights=wts, flags=torch.from_numpy(flags).cuda(), normalise=True)
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy())
+    assert np.all(np.abs(got - Mn) <= 2e-7 * np.abs(Mn))
+    h.destroy()
