@@ -210,35 +210,45 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
     row = cfg.samples_per_input
     data_seconds = cfg.seconds_of_data
 
-    # seeded synthetic voltages, one coarse channel per rank (coarse index = rank), resident in HBM
+    # seeded synthetic voltages, resident in HBM: every rank holds its own cfg.n_coarse coarse channels (weak scaling:
+    # rank r takes coarse indices r, r + world, ...; one channel per GPU for C3/C4, eight for the C5 batch)
+    NCO = cfg.n_coarse
+    mine = shard.coarse_channels_for_rank(world * NCO, rank, world)
     host = torch.empty((1, n, row, 2), dtype=torch.int8).pin_memory()
-    coarse = shard.coarse_channels_for_rank(world, rank, world)[0]   # weak scaling: one coarse channel per GPU
-    synth.gauss_voltages(cfg.spec(coarse=coarse), out=host.numpy()[0])
-    volt = host.cuda()
+    volt = torch.empty((NCO, n, row, 2), dtype=torch.int8, device="cuda")
+    for k, coarse in enumerate(mine):
+        synth.gauss_voltages(cfg.spec(coarse=coarse), out=host.numpy()[0])
+        volt[k].copy_(host[0])
+    torch.cuda.synchronize()
+    data_seconds = data_seconds * NCO
     h = corr.MwaxCorr(n, N, K, T, F)
-    vis = h.new_output(n_dumps=D)
+    vis = h.new_output(n_dumps=D, n_coarse=NCO)
     stream = torch.cuda.current_stream()
     sp = int(stream.cuda_stream)
     dump_bytes = T * N * 2
     L = corr.lib()
 
+    coarse_bytes = n * row * 2
+
     def step(events=None):
-        for d in range(D):
-            if events is not None:
-                e0, e1, e2 = events[d]
-                e0.record(stream)
-            corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr() + d * dump_bytes, row, sp), "f_stage", h._h)
-            if events is not None:
-                e1.record(stream)
-            corr._check(L.mwax_corr_x_stage(h._h, vis[0, d].data_ptr(), sp), "x_stage", h._h)
-            if events is not None:
-                e2.record(stream)
+        for c in range(NCO):
+            for d in range(D):
+                if events is not None:
+                    e0, e1, e2 = events[c * D + d]
+                    e0.record(stream)
+                corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr() + c * coarse_bytes + d * dump_bytes, row, sp),
+                            "f_stage", h._h)
+                if events is not None:
+                    e1.record(stream)
+                corr._check(L.mwax_corr_x_stage(h._h, vis[c, d].data_ptr(), sp), "x_stage", h._h)
+                if events is not None:
+                    e2.record(stream)
 
     for _ in range(warmup):
         step()
     torch.cuda.synchronize()
 
-    evs = [[tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(D)] for _ in range(steps)]
+    evs = [[tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(D * NCO)] for _ in range(steps)]
     sampler = ClockSampler(physical_gpu_index(local_rank))
     if world > 1:
         dist.barrier()
@@ -262,7 +272,7 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
     f_avg_ms, x_avg_ms = sum(f_ms) / len(f_ms), sum(x_ms) / len(x_ms)
     res = {"cfg": cfg, "value": world * data_seconds / (ms_per_step * 1e-3), "ms_per_step": ms_per_step,
            "total_ms": total_ms, "f_ms": f_avg_ms, "x_ms": x_avg_ms, "clocks": clocks,
-           "launches": steps * D * h.launches_per_process(), "in_bytes": host.numel(),
+           "launches": steps * D * NCO * h.launches_per_process(), "in_bytes": volt.numel(),
            "ws_bytes": h.workspace_bytes(), "e2e": None,
            "input_samples_per_s": world * n * row / (ms_per_step * 1e-3)}
 
@@ -298,7 +308,7 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
     del mo
 
     # ---- e2e through the public host-buffer call (H2D + D2H inside the timed region)
-    if do_e2e:
+    if do_e2e and NCO == 1:
         hvis = torch.empty((1, D, C, B, 2), dtype=torch.float32).pin_memory()
         e_steps = max(2, min(steps, 5))
         h.process_host(host, hvis, D, 1)          # warm-up (allocates staging)
@@ -353,7 +363,7 @@ def main():
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C3", "C4"])
+    ap.add_argument("--workload", default="C3", choices=["C3", "C4", "C5"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the second workload reported under 'workloads'")
@@ -377,10 +387,13 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     res = measure(args.workload, args.steps, args.warmup, world, rank, local_rank, not args.no_e2e)
-    other = None
+    others = []
     if not args.no_extra:
-        wl2 = "C4" if args.workload == "C3" else "C3"
-        other = (wl2, measure(wl2, max(3, args.steps // 4), args.warmup, world, rank, local_rank, False))
+        for wl2 in ("C3", "C4", "C5"):
+            if wl2 == args.workload:
+                continue
+            st2 = max(3, args.steps // (32 if wl2 == "C5" else 4))
+            others.append((wl2, st2, measure(wl2, st2, args.warmup, world, rank, local_rank, False)))
 
     if rank == 0:
         peaks = load_peaks()
@@ -393,7 +406,8 @@ def main():
                 "vs_baseline": None, "dtype": "f16 operands, f32 accumulate (FFT in f32)", "data": "synthetic",
                 "config": {"workload": cfg.name, "n_inputs": cfg.n_inputs, "n_fft": cfg.n_fft, "n_keep": cfg.n_keep,
                            "t_int": cfg.t_int, "f_avg": cfg.f_avg, "dumps_per_step": cfg.n_dumps,
-                           "seconds_of_data_per_step": cfg.seconds_of_data, "coarse_channels_per_gpu_per_step": 1,
+                           "seconds_of_data_per_step": cfg.seconds_of_data * cfg.n_coarse,
+                           "coarse_channels_per_gpu_per_step": cfg.n_coarse,
                            "parallelism": f"coarse-channel x{world}",
                            "l2": "inputs larger than L2 (%.2f GB in, %.2f GB workspace per dump)" %
                                  (res["in_bytes"] / 1e9, res["ws_bytes"] / 1e9)},
@@ -406,13 +420,17 @@ def main():
                               "f_stage_ms_with_delay_phase_correction": res.get("f_ms_delay")},
                 "paper_context": "MWAX on 1 x A40 + 2 x Epyc 7F72: 5.9 s per 8 s subfile at 256 tiles, 1 s/10 kHz mode "
                                  "=> 1 coarse channel per GPU in real time (PAPER.md Table 2 L531-545)"}
-        if other is not None:
-            wl2, r2 = other
-            rf2, rx2 = rooflines(r2, peaks, traffic, wl2)
-            line["workloads"] = {r2["cfg"].name: {"value": r2["value"], "ms_per_step": r2["ms_per_step"],
-                                                   "seconds_of_data_per_step": r2["cfg"].seconds_of_data,
-                                                   "steps": max(3, args.steps // 4), "clocks": r2["clocks"],
-                                                   "stages": {"f": rf2, "x": rx2}}}
+        if others:
+            line["workloads"] = {}
+            for wl2, st2, r2 in others:
+                rf2, rx2 = rooflines(r2, peaks, traffic, wl2)
+                line["workloads"][r2["cfg"].name] = {
+                    "value": r2["value"], "ms_per_step": r2["ms_per_step"], "n_inputs": r2["cfg"].n_inputs,
+                    "seconds_of_data_per_step": r2["cfg"].seconds_of_data * r2["cfg"].n_coarse,
+                    "coarse_channels_per_step": r2["cfg"].n_coarse, "steps": st2, "clocks": r2["clocks"],
+                    "stages": {"f": rf2, "x": rx2},
+                    "next_rows": {"mwax_order_ms_per_dump": r2.get("order_ms"),
+                                  "f_stage_ms_with_delay_phase_correction": r2.get("f_ms_delay")}}
         if res["e2e"] is not None:
             line["e2e"] = res["e2e"]
         if not args.no_cpu_baseline and world == 1:

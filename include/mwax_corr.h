@@ -48,7 +48,7 @@ enum {
 };
 
 /* options for mwax_corr_set_option */
-enum { MWAX_OPT_AVG_MODE = 1 };
+enum { MWAX_OPT_AVG_MODE = 1, MWAX_OPT_ACCUMULATE = 2 };
 enum { MWAX_AVG_CENTRE_SYMMETRIC = 0, MWAX_AVG_BLOCK = 1 };
 
 /* ------------------------------------------------------------------------------------------------------
@@ -67,7 +67,12 @@ enum { MWAX_AVG_CENTRE_SYMMETRIC = 0, MWAX_AVG_BLOCK = 1 };
 mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, int f_avg);
 int mwax_corr_last_error(void);
 
-/* Averaging geometry; call before the first process().  Default MWAX_AVG_CENTRE_SYMMETRIC. */
+/* MWAX_OPT_AVG_MODE: averaging geometry; call before the first process().  Default MWAX_AVG_CENTRE_SYMMETRIC (L290).
+ * MWAX_OPT_ACCUMULATE (0/1, default 0): streaming integration (§2.5, §2.5.2:
+ *   50 ms blocks aggregated into the integration).  With 1, process()/process_batch()/x_stage() ADD their result to
+ *   what d_vis already holds, so an integration of any length is the sum of calls over its pieces (t_int = spectra per
+ *   piece, e.g. 10 for one 50 ms block at n_fft = 6400) without keeping the voltages: first piece with 0, the rest
+ *   with 1.  Sums of fp32 partial results; the pieces need not be equal in content but each has t_int spectra. */
 int mwax_corr_set_option(mwax_corr_t *h, int key, int value);
 
 /* Fractional-delay / phase correction (§2.5.1, §2.4.1, §4.3):

@@ -21,6 +21,7 @@ _lib = None
 
 MWAX_OK = 0
 MWAX_OPT_AVG_MODE = 1
+MWAX_OPT_ACCUMULATE = 2
 MWAX_AVG_CENTRE_SYMMETRIC = 0
 MWAX_AVG_BLOCK = 1
 
@@ -124,6 +125,10 @@ class MwaxCorr:
         self.n_baselines = n_inputs * (n_inputs + 1) // 2
         if avg_mode is not None:
             _check(L.mwax_corr_set_option(self._h, MWAX_OPT_AVG_MODE, avg_mode), "mwax_corr_set_option")
+
+    def set_accumulate(self, on: bool):
+        """Streaming integration: with True, process() adds into `vis` instead of overwriting it."""
+        _check(lib().mwax_corr_set_option(self._h, MWAX_OPT_ACCUMULATE, 1 if on else 0), "mwax_corr_set_option", self._h)
 
     # sizes
     def input_bytes(self) -> int:

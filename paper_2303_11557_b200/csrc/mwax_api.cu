@@ -245,6 +245,7 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
 struct mwax_corr {
     int n, N, K, T, F, C;
     int avg_mode;
+    int accumulate;    // MWAX_OPT_ACCUMULATE: process() adds into d_vis
     int x_bn;          // X tile width in G columns (128 or 256)
     int pitch;         // fp16 elements per Y row (2n rounded up to 64)
     int sm_count;
@@ -467,6 +468,11 @@ int mwax_corr_set_option(mwax_corr_t *h, int key, int value)
         h->avg_mode = value;
         return build_tables(h);
     }
+    if (key == MWAX_OPT_ACCUMULATE) {
+        if (value != 0 && value != 1) return MWAX_ERR_INVALID_ARG;
+        h->accumulate = value;
+        return MWAX_OK;
+    }
     return MWAX_ERR_INVALID_ARG;
 }
 
@@ -538,6 +544,7 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
     xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = h->C; xp.n_tiles = h->n_tiles;
     xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = h->n_taps; xp.scale = h->d_scale;
     xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    xp.accumulate = h->accumulate;
     if (h->x_pair) {
         xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
         int rcp = launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
@@ -746,6 +753,7 @@ int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, vo
     xp.n_inputs = h->n; xp.T = h->n_time; xp.K = h->n_chan; xp.n_out = h->n_chan; xp.n_tiles = h->n_tiles;
     xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = 1; xp.scale = nullptr;
     xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    xp.accumulate = 0;
     if (h->x_pair) {
         xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
         rc = launch_x_pair<true>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream);

@@ -34,6 +34,7 @@ struct XParams {
     const float *scale;       // [C] epilogue scale (float path only)
     void *out;                // float2 / int2 [C][n(n+1)/2]
     long long out_chan_stride;  // n(n+1)/2
+    int accumulate;             // float path: add to what `out` already holds (integration across calls) instead of overwriting
 };
 
 template <bool kInt8, int BN>
@@ -101,6 +102,11 @@ __device__ __forceinline__ void x_epilogue_tile(const XParams &P, float *stg, ui
             if (i < n && j <= i) {
                 if (i == j) v.y = 0.0f;       // autos: Im := 0 exactly (int path: bit pattern 0 as well)
                 const long long o = (long long)c * P.out_chan_stride + ((long long)i * (i + 1) / 2 + j);
+                if (!kInt8 && P.accumulate) {
+                    const float2 old = reinterpret_cast<const float2 *>(P.out)[o];
+                    v.x += old.x;
+                    v.y += old.y;
+                }
                 reinterpret_cast<float2 *>(P.out)[o] = v;
             }
         }

@@ -412,3 +412,33 @@ def test_occupancy_weights_and_normalisation(n, C, S):
     got = _complex(out.cpu().numpy())
     assert np.all(np.abs(got - Mn) <= 2e-7 * np.abs(Mn))
     h.destroy()
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# streaming integration over the paper's block structure (PAPER.md 2.5 L258, 2.5.2 L280)
+# ------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("n,N,F,spb,blocks", [
+    (16, 64, 1, 8, 5),           # five blocks of 8 spectra
+    (12, 6400, 50, 10, 3),       # the paper's shape: 50 ms blocks of 10 x 6400-point frames, fscrunch 50
+])
+def test_streaming_accumulation_over_blocks_equals_one_integration(n, N, F, spb, blocks):
+    """Subfile-shaped input [block][input][spb*N] fed one block per call with MWAX_OPT_ACCUMULATE equals the oracle's
+    single integration over all blocks (the oracle's additivity over time is pinned in test_p4_additivity_over_time)."""
+    T = spb * blocks
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.25, tones=[synth.Tone(3, 5.0, 1)], seed=555 + N)
+    volt = synth.gauss_voltages(spec)                                        # [n][T*N][2]
+    ref = oracle.fx(volt, N, N, T, F)
+    sub = np.ascontiguousarray(volt.reshape(n, blocks, spb * N, 2).transpose(1, 0, 2, 3))   # [block][input][spb*N][2] (L258-260)
+    h = corr.MwaxCorr(n, N, N, spb, F)
+    vis = h.new_output()[0, 0]
+    vis.fill_(float("nan"))
+    dsub = torch.from_numpy(sub).cuda()
+    for b in range(blocks):
+        h.set_accumulate(b > 0)
+        h.process(dsub[b], vis)
+    torch.cuda.synchronize()
+    got = _complex(vis.cpu().numpy())
+    assert _norm_err(got, ref, n) <= TOL
+    ii = np.arange(n)
+    assert np.all(got[:, ii * (ii + 1) // 2 + ii].imag == 0.0)
+    h.destroy()
