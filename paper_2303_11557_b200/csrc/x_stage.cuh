@@ -12,10 +12,13 @@
 // Z's layout [row][2n] makes both operands MN-major (the contraction index is the slow axis): TMA (SWIZZLE_128B)
 // drops 128-byte x BK-row boxes into shared memory in exactly the canonical MN-major UMMA layout.
 //
-// Kernel shape: persistent CTAs, 6 warps: warp 0 = TMA producer, warp 1 = MMA issuer (+ TMEM owner),
-// warps 2..5 = epilogue (TMEM lanes 32*(warp%4)..+31).  A work item is (output channel c, G-tile (mi, nj)):
-// a 128 x BN fp32/int32 accumulator in TMEM, double buffered so the epilogue of one item overlaps the MMAs of
-// the next.  Work items are ordered channel-major so concurrently running CTAs share a channel's rows in L2.
+// This file: the SINGLE-CTA kernel (tcgen05 cta_group::1; selected with MWAX_X_PAIR=0, the cross-check of the CTA-pair
+// kernel in x_stage2.cuh, which is the default) and the epilogue both kernels share.
+// Kernel shape: persistent CTAs, 6 warps: warp 0 = TMA producer (one lane), warp 1 = MMA issuer (+ TMEM owner; all
+// lanes run the loops, one elected lane issues), warps 2..5 = epilogue (TMEM lanes 32*(warp%4)..+31).  A work item is
+// (output channel c, G-tile): a 128 x 256 (128 x 128 on the diagonal) fp32/int32 accumulator in TMEM, double buffered
+// so the epilogue of one item overlaps the MMAs of the next.  Work items are ordered channel-major so concurrently
+// running CTAs share a channel's rows in L2.
 #pragma once
 #include <cuda_fp16.h>
 #include "ptx.cuh"
