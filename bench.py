@@ -196,7 +196,7 @@ def load_traffic():
     return out
 
 
-def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
+def measure(wl, steps, warmup, world, rank, local_rank, do_e2e, do_next=True):
     """Time `steps` passes of the whole hot path over workload `wl` (device-resident input), per-stage CUDA events
     inside the timed region, then the end-to-end leg through mwax_corr_process_host."""
     import torch
@@ -277,35 +277,36 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e):
            "input_samples_per_s": world * n * row / (ms_per_step * 1e-3)}
 
     # ---- F stage with the fractional-delay / phase correction switched on
-    g = torch.Generator(device="cuda").manual_seed(1234 + rank)
-    dly = (torch.rand((n, T * D), generator=g, device="cuda") - 0.5).float().contiguous()
-    phs = ((torch.rand((n, T * D), generator=g, device="cuda") - 0.5) * 6.0).float().contiguous()
-    h.set_delays(dly, phs)
-    for _ in range(2):
-        corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr(), row, sp), "f_stage", h._h)
-    d0 = torch.cuda.Event(enable_timing=True)
-    d1 = torch.cuda.Event(enable_timing=True)
-    n_rep = 10
-    d0.record(stream)
-    for _ in range(n_rep):
-        corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr(), row, sp), "f_stage", h._h)
-    d1.record(stream)
-    torch.cuda.synchronize()
-    res["f_ms_delay"] = d0.elapsed_time(d1) / n_rep
-    h.set_delays(None, None)
+    if do_next:
+        g = torch.Generator(device="cuda").manual_seed(1234 + rank)
+        dly = (torch.rand((n, T * D), generator=g, device="cuda") - 0.5).float().contiguous()
+        phs = ((torch.rand((n, T * D), generator=g, device="cuda") - 0.5) * 6.0).float().contiguous()
+        h.set_delays(dly, phs)
+        for _ in range(2):
+            corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr(), row, sp), "f_stage", h._h)
+        d0 = torch.cuda.Event(enable_timing=True)
+        d1 = torch.cuda.Event(enable_timing=True)
+        n_rep = 10
+        d0.record(stream)
+        for _ in range(n_rep):
+            corr._check(L.mwax_corr_f_stage(h._h, volt.data_ptr(), row, sp), "f_stage", h._h)
+        d1.record(stream)
+        torch.cuda.synchronize()
+        res["f_ms_delay"] = d0.elapsed_time(d1) / n_rep
+        h.set_delays(None, None)
 
-    # ---- MWAX_ORDER emitter on one dump (PAPER.md 2.7: 0.6-1.8 s of CPU time per 8 s in Table 2)
-    mo = h.to_mwax_order(vis[0, 0])
-    o0 = torch.cuda.Event(enable_timing=True)
-    o1 = torch.cuda.Event(enable_timing=True)
-    o0.record(stream)
-    for _ in range(n_rep):
-        h.to_mwax_order(vis[0, 0], mo)
-    o1.record(stream)
-    torch.cuda.synchronize()
-    res["order_ms"] = o0.elapsed_time(o1) / n_rep
-    res["order_gbs"] = (vis[0, 0].numel() * 4 + mo.numel() * 4) / (res["order_ms"] * 1e-3) / 1e9
-    del mo
+        # ---- MWAX_ORDER emitter on one dump (PAPER.md 2.7: 0.6-1.8 s of CPU time per 8 s in Table 2)
+        mo = h.to_mwax_order(vis[0, 0])
+        o0 = torch.cuda.Event(enable_timing=True)
+        o1 = torch.cuda.Event(enable_timing=True)
+        o0.record(stream)
+        for _ in range(n_rep):
+            h.to_mwax_order(vis[0, 0], mo)
+        o1.record(stream)
+        torch.cuda.synchronize()
+        res["order_ms"] = o0.elapsed_time(o1) / n_rep
+        res["order_gbs"] = (vis[0, 0].numel() * 4 + mo.numel() * 4) / (res["order_ms"] * 1e-3) / 1e9
+        del mo
 
     # ---- e2e through the public host-buffer call (H2D + D2H inside the timed region)
     if do_e2e and NCO == 1:
@@ -366,7 +367,8 @@ def main():
     ap.add_argument("--workload", default="C3", choices=["C3", "C4", "C5"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-extra", action="store_true", help="skip the second workload reported under 'workloads'")
+    ap.add_argument("--no-extra", action="store_true", help="skip the other workloads reported under 'workloads'")
+    ap.add_argument("--no-next-rows", action="store_true", help="skip the delay-correction and MWAX_ORDER timings")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else max(args.warmup, 0)
 
@@ -386,14 +388,14 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
-    res = measure(args.workload, args.steps, args.warmup, world, rank, local_rank, not args.no_e2e)
+    res = measure(args.workload, args.steps, args.warmup, world, rank, local_rank, not args.no_e2e, not args.no_next_rows)
     others = []
     if not args.no_extra:
         for wl2 in ("C3", "C4", "C5"):
             if wl2 == args.workload:
                 continue
             st2 = max(3, args.steps // (32 if wl2 == "C5" else 4))
-            others.append((wl2, st2, measure(wl2, st2, args.warmup, world, rank, local_rank, False)))
+            others.append((wl2, st2, measure(wl2, st2, args.warmup, world, rank, local_rank, False, not args.no_next_rows)))
 
     if rank == 0:
         peaks = load_peaks()
