@@ -161,16 +161,9 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
         const int i = ((item - t * groups) * Q + (int)rank) * C::G + g;
         if (item < n_items && i < P.n_inputs) {
             const int8_t *src = P.volt + 2 * ((long long)i * P.row_pitch + P.sample0 + (long long)t * C::N + 16 * hi + 2 * lo);
-            if (P.vec_ok) {
 #pragma unroll
-                for (int q = 0; q < 20; ++q) raw[q] = __ldg(reinterpret_cast<const unsigned *>(src + 640 * q));
-            } else {
-#pragma unroll
-                for (int q = 0; q < 20; ++q) {
-                    const unsigned short *s16 = reinterpret_cast<const unsigned short *>(src + 640 * q);
-                    raw[q] = (uint32_t)__ldg(s16) | ((uint32_t)__ldg(s16 + 1) << 16);
-                }
-            }
+            for (int q = 0; q < 20; ++q) raw[q] = __ldg(reinterpret_cast<const unsigned *>(src + 640 * q));   // 4-byte aligned: the
+                                                                     // plan sends misaligned buffers to the generic kernel
         } else {
 #pragma unroll
             for (int q = 0; q < 20; ++q) raw[q] = 0u;                // absent input: zeros

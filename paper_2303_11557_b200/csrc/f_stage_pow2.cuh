@@ -148,17 +148,9 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
             q[v] = make_int4(0, 0, 0, 0);
             if (rok[v]) {
                 const int8_t *s = src[v] + 2ll * t * N;
-                if (P.vec_ok) {
-                    q[v] = __ldg(reinterpret_cast<const int4 *>(s));
-                } else {
-                    const uint16_t *s16 = reinterpret_cast<const uint16_t *>(s);   // samples are 2-byte aligned
-                    uint32_t ww[4];
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) ww[e] = (uint32_t)s16[2 * e] | ((uint32_t)s16[2 * e + 1] << 16);
-                    q[v] = make_int4((int)ww[0], (int)ww[1], (int)ww[2], (int)ww[3]);
-                }
-            }
-        }
+                q[v] = __ldg(reinterpret_cast<const int4 *>(s));   // rows are 16-byte aligned here: the plan sends anything
+            }                                                  // else to the generic kernel (a predicated scalar path
+        }                                                      // would cost an issue slot per sample even when unused)
     };
     auto stash = [&](const int4 (&q)[C::VPT]) {
 #pragma unroll
@@ -189,7 +181,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
     const int i = i0 + lane;
     const bool iok = i < P.n_inputs;
     const int half = P.K / 2;
-    const size_t chan_stride = (size_t)P.T * P.pitch2;                // half2 elements between positions
+    const unsigned chan_stride = (unsigned)P.T * (unsigned)P.pitch2;  // half2 elements between positions (< 2^32: checked at create)
     __half2 *ybase = P.Y + i;
 
     for (int t = t_begin; t < t_end; ++t) {
@@ -259,8 +251,8 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
                             v.x *= f;
                             v.y *= f;
                         }
-                        __half2 *dst = (k2 < R2 / 2) ? yp + (size_t)(R1 * k2) * chan_stride
-                                                     : yn + (size_t)(R1 * (k2 - R2 / 2)) * chan_stride;
+                        __half2 *dst = (k2 < R2 / 2) ? yp + (size_t)(unsigned)(R1 * k2) * chan_stride      // one IMAD.WIDE.U32
+                                                     : yn + (size_t)(unsigned)(R1 * (k2 - R2 / 2)) * chan_stride;
                         *dst = __floats2half2_rn(v.x, v.y);
                     }
                 }

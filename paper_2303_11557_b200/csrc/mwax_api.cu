@@ -228,14 +228,21 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
     }
     const int n_items = xp.n_out * xp.n_tiles;
     if (n_items <= 0) return MWAX_OK;
-    int pairs = sm_count / 2;
-    if (n_items < pairs) pairs = n_items;
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.gridDim = dim3(2 * pairs); cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
+    cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
     cfg.attrs = attr; cfg.numAttrs = 1;
+    static int max_pairs = 0;          // pairs the device can hold at once (GPCs with an odd SM count leave one SM unpaired)
+    if (!max_pairs) {
+        cfg.gridDim = dim3(2);
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = sm_count / 2;
+        max_pairs = n < sm_count / 2 ? n : sm_count / 2;
+    }
+    const int pairs = n_items < max_pairs ? n_items : max_pairs;   // persistent: never more pairs than run concurrently
+    cfg.gridDim = dim3(2 * pairs);
     return cudaLaunchKernelEx(&cfg, kern, tmap, tmap_flat, xp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
 }
 
@@ -414,6 +421,9 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     if (const char *e = getenv("MWAX_X_TILE_N")) { if (atoi(e) == 128) h->x_bn = 128; }
     h->x_pair = want_pair_kernel();
     h->pitch = ((2 * n_inputs + 63) / 64) * 64;
+    if ((unsigned long long)t_int * (unsigned long long)(h->pitch / 2) >= (1ull << 32)) {   // kernels keep this stride in 32 bits
+        g_last_error = MWAX_ERR_UNSUPPORTED; delete h; return nullptr;
+    }
     h->sm_count = sm;
     h->last_cuda = 0;
     h->radix = radix;
@@ -427,7 +437,8 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     if (const char *e = getenv("MWAX_F_GENERIC")) { if (atoi(e) == 1) n_fft = -n_fft; }
     cudaError_t ae = cudaSuccess;
     if (n_fft == 64 || n_fft == 128 || n_fft == 256 || n_fft == 512 || n_fft == 6400) h->f_kind = n_fft;
-    else ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
+    // the generic kernel also serves the specialised lengths when a buffer is not 16-byte aligned
+    ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
     if (n_fft < 0) n_fft = -n_fft;
     if (ae != cudaSuccess) { g_last_error = MWAX_ERR_CUDA; delete h; return nullptr; }
     // twiddles exp(-2 pi i m / N), computed in double
@@ -494,12 +505,13 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
     fp.d_stride = (long long)h->d_row_stride; fp.frame0 = frame0;
     fp.y_p_stride = (unsigned)h->T * (unsigned)(h->pitch / 2); fp.y_t_stride = (unsigned)(h->pitch / 2);
     cudaStream_t st = (cudaStream_t)stream;
-    if (h->f_kind == 6400) {
+    const int f_kind = fp.vec_ok ? h->f_kind : 0;          // misaligned rows: generic kernel (scalar loads)
+    if (f_kind == 6400) {
         const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
         int rc = h->f_p3 == 8 ? launch_f_6400p3<8>(fp, full, scale, delay, st) : h->f_p3 == 4 ? launch_f_6400p3<4>(fp, full, scale, delay, st)
                                                                         : launch_f_6400p3<2>(fp, full, scale, delay, st);
         if (rc != MWAX_OK) return rc;
-    } else if (h->f_kind) {
+    } else if (f_kind) {
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
         const int groups = (h->n + 31) / 32;
         long long fpc = ((long long)groups * h->T) / ((long long)h->sm_count * 24);
@@ -509,7 +521,7 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
         const int chunks = (h->T + (int)fpc - 1) / (int)fpc;
         const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
         int rc;
-        switch (h->f_kind) {
+        switch (f_kind) {
             case 64: rc = launch_f_pow2<64, 8, 16>(fp, full, scale, delay, groups, chunks, st); break;
             case 128: rc = launch_f_pow2<128, 8, 16>(fp, full, scale, delay, groups, chunks, st); break;
             case 256: rc = launch_f_pow2<256, 16, 32>(fp, full, scale, delay, groups, chunks, st); break;
