@@ -333,6 +333,40 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e, do_next=True):
     return res
 
 
+def measure_c2(steps, warmup):
+    """BASELINE.json configs[1]: X-only integer path, 512 inputs x 1024 pre-channelised fine channels x 2000 samples,
+    int8 in / int32 out, device-resident (the bit-exactness of this path is a parity test, not repeated here)."""
+    import torch
+    from paper_2303_11557_b200 import corr, synth
+    n, n_chan, n_time = 512, 1024, 2000
+    host = torch.empty((n_chan, n_time, n, 2), dtype=torch.int8).pin_memory()
+    synth.uniform_voltages(n_chan, n_time, n, n_shared=64, out=host.numpy())
+    z = host.cuda()
+    del host
+    h = corr.MwaxXcorrI8(n, n_chan, n_time)
+    out = h.new_output()
+    stream = torch.cuda.current_stream()
+    for _ in range(warmup):
+        h.process(z, out)
+    torch.cuda.synchronize()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        h.process(z, out)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    B = n * (n + 1) // 2
+    ops = 8.0 * B * n_chan * n_time                       # same count as the float path: 8 real ops per complex MAC
+    res = {"ms_per_launch": ms, "tops_algorithmic": ops / (ms * 1e-3) / 1e12, "bytes_in": z.numel(),
+           "bytes_out": out.numel() * 4, "hbm_gbs_algorithmic": (z.numel() + out.numel() * 4) / (ms * 1e-3) / 1e9}
+    h.destroy()
+    del z, out
+    torch.cuda.empty_cache()
+    return res
+
+
 def rooflines(res, peaks, traffic, wl):
     """F stage = 6 bytes per kept input sample against HBM; X stage = 8 n(n+1)/2 flops per
     (fine channel, time) sample against the dense 16-bit tensor peak."""
@@ -363,7 +397,8 @@ def main():
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="C3", choices=["C3", "C4", "C5"])
+    ap.add_argument("--workload", default="C3", choices=["C3", "C4", "C5", "C2"],
+                    help="C3 (default, headline) / C4 / C5: the FX path; C2: the X-only int8 path alone (own metric)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-extra", action="store_true", help="skip the other workloads reported under 'workloads'")
@@ -387,6 +422,19 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
+    if args.workload == "C2":      # the integer X-only path on its own (used for its ncu capture): a different metric
+        c2 = measure_c2(args.steps, args.warmup)
+        if rank == 0:
+            peaks = load_peaks()
+            print(json.dumps({"metric": "x_only_int8_tera_ops_per_s", "value": c2["tops_algorithmic"], "unit": "TOP/s",
+                              "n_gpus": 1, "steps": args.steps, "warmup": args.warmup, "ms_per_step": c2["ms_per_launch"],
+                              "higher_is_better": True, "dtype": "s8 operands, s32 accumulate", "data": "synthetic",
+                              "config": {"workload": "C2-xonly-int8", "n_inputs": 512, "n_chan": 1024, "n_time": 2000},
+                              "gpu_launches": args.steps,
+                              "roofline": {"bound": "tensor", "achieved": c2["tops_algorithmic"], "unit": "TOP/s",
+                                           "peak": 2.0 * peaks["tensor_burst"], "frac": c2["tops_algorithmic"] / (2.0 * peaks["tensor_burst"]),
+                                           "traffic": None, "peak_source": "2 x measured bf16 burst"}}), flush=True)
+        return
     res = measure(args.workload, args.steps, args.warmup, world, rank, local_rank, not args.no_e2e, not args.no_next_rows)
     others = []
     if not args.no_extra:
@@ -395,6 +443,7 @@ def main():
                 continue
             st2 = max(3, args.steps // (32 if wl2 == "C5" else 4))
             others.append((wl2, st2, measure(wl2, st2, args.warmup, world, rank, local_rank, False, not args.no_next_rows)))
+    c2 = measure_c2(20, args.warmup) if (not args.no_extra and rank == 0) else None
 
     if rank == 0:
         peaks = load_peaks()
@@ -432,6 +481,15 @@ def main():
                     "stages": {"f": rf2, "x": rx2},
                     "next_rows": {"mwax_order_ms_per_dump": r2.get("order_ms"),
                                   "f_stage_ms_with_delay_phase_correction": r2.get("f_ms_delay")}}
+        if c2 is not None:
+            int8_peak = 2.0 * peaks["tensor_burst"]          # measured bf16 peak x the guide's nominal int8 : bf16 ratio (4.5 : 2.25)
+            line.setdefault("workloads", {})["C2-xonly-int8"] = {
+                "kernel": "x_stage_pair_kernel<int8>", "ms_per_launch": c2["ms_per_launch"],
+                "tensor": {"achieved": c2["tops_algorithmic"], "unit": "TOP/s", "peak": int8_peak,
+                           "frac": c2["tops_algorithmic"] / int8_peak, "peak_source": "2 x measured bf16 burst"},
+                "hbm": {"achieved": c2["hbm_gbs_algorithmic"], "unit": "GB/s", "peak": peaks["hbm_gbs"],
+                        "frac": c2["hbm_gbs_algorithmic"] / peaks["hbm_gbs"]},
+                "note": "tensor and HBM co-bound by construction: 2.10 GB in + 1.08 GB out per 2.15 Tera-ops (SURVEY 8(d))"}
         if res["e2e"] is not None:
             line["e2e"] = res["e2e"]
         if not args.no_cpu_baseline and world == 1:
