@@ -443,3 +443,22 @@ def test_streaming_accumulation_over_blocks_equals_one_integration(n, N, F, spb,
     ii = np.arange(n)
     assert np.all(got[:, ii * (ii + 1) // 2 + ii].imag == 0.0)
     h.destroy()
+
+
+@pytest.mark.parametrize("n,N,T,F", [(20, 128, 6, 1), (8, 6400, 2, 50)])
+def test_misaligned_voltage_buffer_takes_the_scalar_load_path(n, N, T, F):
+    """A buffer that is only 2-byte aligned (samples are 2 bytes) is legal: the plan routes it to the generic kernel
+    instead of the 16-byte-load kernels; results must not change."""
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[synth.Tone(3, 6.0, 1)], seed=321 + N)
+    volt = synth.gauss_voltages(spec)
+    ref = oracle.fx(volt, N, N, T, F)
+    flat = torch.zeros(volt.size + 64, dtype=torch.int8, device="cuda")
+    view = flat[2:2 + volt.size].view(n, N * T, 2)
+    view.copy_(torch.from_numpy(volt))
+    assert view.data_ptr() % 16 == 2 and view.is_contiguous()
+    h = corr.MwaxCorr(n, N, N, T, F)
+    out = h.new_output()[0, 0]
+    h.process(view, out)
+    torch.cuda.synchronize()
+    assert _norm_err(_complex(out.cpu().numpy()), ref, n) <= TOL
+    h.destroy()
