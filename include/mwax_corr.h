@@ -143,6 +143,10 @@ int mwax_corr_to_mwax_order_weighted(mwax_corr_t *h, const float *d_vis, const u
 size_t mwax_corr_input_bytes(const mwax_corr_t *h);
 size_t mwax_corr_output_bytes(const mwax_corr_t *h);
 size_t mwax_corr_workspace_bytes(const mwax_corr_t *h);
+/* Caller-owned workspace (e.g. a torch tensor) instead of the one create() allocated: d_ws is DEVICE memory of at
+ * least mwax_corr_workspace_bytes() bytes, 256-byte aligned; it is zeroed here, the library's own buffer is released,
+ * and the memory must outlive the handle's last call.  Synchronises the device; not to be called with work in flight. */
+int mwax_corr_set_workspace(mwax_corr_t *h, void *d_ws, size_t bytes);
 /* number of kernel launches one process() call enqueues */
 int mwax_corr_launches_per_process(const mwax_corr_t *h);
 int mwax_corr_last_cuda_error(const mwax_corr_t *h);

@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.mwax_corr_process_host.argtypes = [vp, vp, sz, sz, i32, i32, vp, vp]
         L.mwax_corr_f_stage.argtypes = [vp, vp, sz, vp]
         L.mwax_corr_set_delays.argtypes = [vp, vp, vp, sz, sz]
+        L.mwax_corr_set_workspace.argtypes = [vp, vp, sz]
         L.mwax_corr_to_mwax_order.argtypes = [vp, vp, vp, vp, vp]
         L.mwax_corr_to_mwax_order_weighted.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
         L.mwax_corr_mwax_order_bytes.restype = sz
@@ -125,6 +126,13 @@ class MwaxCorr:
         self.n_baselines = n_inputs * (n_inputs + 1) // 2
         if avg_mode is not None:
             _check(L.mwax_corr_set_option(self._h, MWAX_OPT_AVG_MODE, avg_mode), "mwax_corr_set_option")
+
+    def set_workspace(self, ws: torch.Tensor):
+        """Use a caller-owned CUDA tensor (>= workspace_bytes(), 256-byte aligned) as the fp16 spectra workspace."""
+        assert ws.is_cuda and ws.is_contiguous()
+        self._ws_ref = ws
+        _check(lib().mwax_corr_set_workspace(self._h, ws.data_ptr(), ws.numel() * ws.element_size()), "mwax_corr_set_workspace",
+               self._h)
 
     def set_accumulate(self, on: bool):
         """Streaming integration: with True, process() adds into `vis` instead of overwriting it."""

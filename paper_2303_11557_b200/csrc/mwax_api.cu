@@ -277,6 +277,7 @@ struct mwax_corr {
     int n_ptiles, x_pair;
     int n_tiles, n_taps;
     __half *d_Y;
+    bool y_owned;      // false after mwax_corr_set_workspace: the caller owns the memory
     size_t y_bytes;
     CUtensorMap tmap;       // Y as [p][t][2n]: one channel position per box (rows past T read as zero)
     CUtensorMap tmap_flat;  // Y as [p T + t][2n]: boxes may run across adjacent channel positions
@@ -457,6 +458,7 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     if (cudaMalloc(reinterpret_cast<void **>(&h->d_Y), h->y_bytes) != cudaSuccess) {
         g_last_error = MWAX_ERR_NOMEM; mwax_corr_destroy(h); return nullptr;
     }
+    h->y_owned = true;
     cudaMemset(h->d_Y, 0, h->y_bytes);
     if ((g_last_error = encode_z_map(&h->tmap, false, h->d_Y, (uint64_t)h->pitch, (uint64_t)h->pitch * 2,
                                      (uint64_t)t_int, (uint64_t)n_keep, 64)) != MWAX_OK) {
@@ -673,6 +675,22 @@ size_t mwax_corr_output_bytes(const mwax_corr_t *h)
 {
     return h ? (size_t)h->C * ((size_t)h->n * (h->n + 1) / 2) * 8 : 0;
 }
+int mwax_corr_set_workspace(mwax_corr_t *h, void *d_ws, size_t bytes)
+{
+    if (!h || !d_ws) return MWAX_ERR_NULL;
+    if (bytes < h->y_bytes || (reinterpret_cast<uintptr_t>(d_ws) & 255u)) return MWAX_ERR_INVALID_ARG;
+    if (cudaMemset(d_ws, 0, h->y_bytes) != cudaSuccess) return note_cuda(&h->last_cuda);   // pad columns must read as zero
+    int rc = encode_z_map(&h->tmap, false, d_ws, (uint64_t)h->pitch, (uint64_t)h->pitch * 2, (uint64_t)h->T, (uint64_t)h->K, 64);
+    if (rc == MWAX_OK)
+        rc = encode_z_map(&h->tmap_flat, false, d_ws, (uint64_t)h->pitch, (uint64_t)h->pitch * 2, (uint64_t)h->T * h->K, 1, 64);
+    if (rc != MWAX_OK) return rc;
+    if (cudaDeviceSynchronize() != cudaSuccess) return note_cuda(&h->last_cuda);
+    if (h->y_owned) cudaFree(h->d_Y);
+    h->d_Y = reinterpret_cast<__half *>(d_ws);
+    h->y_owned = false;
+    return MWAX_OK;
+}
+
 size_t mwax_corr_mwax_order_bytes(const mwax_corr_t *h)
 {
     if (!h || (h->n & 1)) return 0;
@@ -710,7 +728,7 @@ int mwax_corr_destroy(mwax_corr_t *h)
     if (!h) return MWAX_OK;
     free_tables(h);
     cudaFree(h->d_tw);
-    cudaFree(h->d_Y);
+    if (h->y_owned) cudaFree(h->d_Y);
     cudaFree(h->d_in);
     cudaFree(h->d_out);
     for (cudaEvent_t e : h->ev_in) cudaEventDestroy(e);

@@ -462,3 +462,21 @@ def test_misaligned_voltage_buffer_takes_the_scalar_load_path(n, N, T, F):
     torch.cuda.synchronize()
     assert _norm_err(_complex(out.cpu().numpy()), ref, n) <= TOL
     h.destroy()
+
+
+def test_caller_owned_workspace_gives_the_same_result():
+    n, N, T, F = 24, 128, 30, 4
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[], seed=77)
+    volt = synth.gauss_voltages(spec)
+    ref = oracle.fx(volt, N, N, T, F)
+    h = corr.MwaxCorr(n, N, N, T, F)
+    ws = torch.full((h.workspace_bytes() + 512,), 0x7F, dtype=torch.uint8, device="cuda")     # garbage: must be zeroed by the call
+    off = (-ws.data_ptr()) % 256
+    h.set_workspace(ws[off:off + h.workspace_bytes()])
+    out = h.new_output()[0, 0]
+    h.process(torch.from_numpy(volt).cuda(), out)
+    torch.cuda.synchronize()
+    assert _norm_err(_complex(out.cpu().numpy()), ref, n) <= TOL
+    with pytest.raises(corr.MwaxError):
+        h.set_workspace(ws[off:off + 16])                                                      # too small
+    h.destroy()
