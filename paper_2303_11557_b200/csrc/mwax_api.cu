@@ -241,7 +241,8 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
         if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = sm_count / 2;
         max_pairs = n < sm_count / 2 ? n : sm_count / 2;
     }
-    const int pairs = n_items < max_pairs ? n_items : max_pairs;   // persistent: never more pairs than run concurrently
+    int pairs = n_items < max_pairs ? n_items : max_pairs;   // persistent: never more pairs than run concurrently
+    if (const char *e = getenv("MWAX_X_PAIRS")) { const int v = atoi(e); if (v >= 1 && v < pairs) pairs = v; }
     cfg.gridDim = dim3(2 * pairs);
     return cudaLaunchKernelEx(&cfg, kern, tmap, tmap_flat, xp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
 }

@@ -98,8 +98,11 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
             int s = 0;
             uint32_t ph = 0;
             auto load_block = [&](const CUtensorMap *m, int mi, int nj, int row, int chan) {
+                // diagonal tile: this CTA's half of B (columns 256 nj + 128 r ..) IS its A operand (rows 256 mi + 128 r ..):
+                // loaded once, the MMA's B descriptor points at the A bytes (a fifth less L2 -> SM traffic at n = 512)
+                const bool diag = (mi == nj);
                 ptx::mbar_wait(empty_bar(s), ph ^ 1u);
-                if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(s), 2u * C::STAGE_BYTES);   // both CTAs' bytes
+                if (rank == 0) ptx::mbar_arrive_expect_tx(full_bar(s), diag ? 2u * C::A_BYTES : 2u * C::STAGE_BYTES);   // both CTAs' bytes
                 const uint32_t lead_full = ptx::mapa(full_bar(s), 0);
                 const uint32_t a_dst = stage_base + s * C::STAGE_BYTES;
                 const uint32_t b_dst = a_dst + C::A_BYTES;
@@ -107,10 +110,12 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
                 for (int ch = 0; ch < C::CHUNKS; ++ch)
                     ptx::tma_load_3d_pair(a_dst + ch * C::CHUNK_BYTES, m, mi * 256 + (int)rank * 128 + ch * C::CHUNK_ELEMS, row,
                                           chan, lead_full);
+                if (!diag) {
 #pragma unroll
-                for (int ch = 0; ch < C::CHUNKS; ++ch)
-                    ptx::tma_load_3d_pair(b_dst + ch * C::CHUNK_BYTES, m, nj * 256 + (int)rank * 128 + ch * C::CHUNK_ELEMS, row,
-                                          chan, lead_full);
+                    for (int ch = 0; ch < C::CHUNKS; ++ch)
+                        ptx::tma_load_3d_pair(b_dst + ch * C::CHUNK_BYTES, m, nj * 256 + (int)rank * 128 + ch * C::CHUNK_ELEMS, row,
+                                              chan, lead_full);
+                }
                 if (++s == C::STAGES) { s = 0; ph ^= 1u; }
             };
             for (int item = pair; item < n_items; item += n_pairs) {
@@ -144,13 +149,13 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
             uint32_t ph = 0;
             int as = 0;
             uint32_t aph = 0;
-            uint32_t d_tmem = 0, accumulate = 0;
+            uint32_t d_tmem = 0, accumulate = 0, b_off = C::A_BYTES;
             auto mma_block = [&](int rows) {
                 ptx::mbar_wait(full_bar(s), ph);
                 ptx::tc_fence_after();
                 const uint32_t a_src = stage_base + s * C::STAGE_BYTES;
                 if (ptx::elect_one()) {
-                    ptx::mma_block_issue<kInt8, true, C::BK, C::KINST>(a_src, a_src + C::A_BYTES, C::CHUNK_BYTES, d_tmem, C::IDESC,
+                    ptx::mma_block_issue<kInt8, true, C::BK, C::KINST>(a_src, a_src + b_off, C::CHUNK_BYTES, d_tmem, C::IDESC,
                                                                         rows, accumulate);
                     ptx::tc_commit_pair(empty_bar(s), 3);   // frees slot s in BOTH CTAs when these MMAs have read it
                 }
@@ -160,6 +165,8 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
             };
             for (int item = pair; item < n_items; item += n_pairs) {
                 const int c = item / P.n_tiles;
+                const int tile = item - c * P.n_tiles;
+                b_off = (P.tiles[4 * tile] == P.tiles[4 * tile + 1]) ? 0u : (uint32_t)C::A_BYTES;   // diagonal tile: B = A
                 ptx::mbar_wait(tempty_bar(as), aph ^ 1u);
                 ptx::tc_fence_after();
                 d_tmem = tmem_base + (uint32_t)(as * C::BN);
