@@ -45,6 +45,41 @@ __device__ __forceinline__ float2 cmul(float2 a, float2 b)
     return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
 }
 
+// Packed fp32 pairs (sm_100 add/sub/fma .f32x2 -> FADD2 / FFMA2): one issue slot for the real and the imaginary part.
+// The F kernels are issue bound, not FP32-lane bound (profiles/r1_ncu_full.md), so complex adds and subtractions, which
+// are most of an FFT's instructions, go through these.  Same IEEE round-to-nearest results as the scalar forms.
+__device__ __forceinline__ unsigned long long pack2(float2 a)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+    return r;
+}
+__device__ __forceinline__ float2 unpack2(unsigned long long r)
+{
+    float2 a;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+    return a;
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
+    return unpack2(r);
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b)
+{
+    unsigned long long r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
+    return unpack2(r);
+}
+// (a.x * b.x + c.x, a.y * b.y + c.y)
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
+{
+    unsigned long long r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)), "l"(pack2(c)));
+    return unpack2(r);
+}
+
 // Delay/phase gain of one (input, frame): applying a delay of d samples multiplies signed bin u by
 // exp(i (phase - 2 pi u d / N)) (shift theorem; reading Q19).  Kept in TURNS so that the argument of the
 // fast sine/cosine is reduced exactly: turns(u) = pt + u * st, pt = phase / 2 pi, st = -d / N.
@@ -75,18 +110,18 @@ template <>
 __device__ __forceinline__ void butterfly<2>(float2 (&x)[2])
 {
     const float2 a = x[0], b = x[1];
-    x[0] = make_float2(a.x + b.x, a.y + b.y);
-    x[1] = make_float2(a.x - b.x, a.y - b.y);
+    x[0] = cadd(a, b);
+    x[1] = csub(a, b);
 }
 template <>
 __device__ __forceinline__ void butterfly<4>(float2 (&x)[4])
 {
-    const float2 a = make_float2(x[0].x + x[2].x, x[0].y + x[2].y);
-    const float2 b = make_float2(x[0].x - x[2].x, x[0].y - x[2].y);
-    const float2 c = make_float2(x[1].x + x[3].x, x[1].y + x[3].y);
-    const float2 d = make_float2(x[1].x - x[3].x, x[1].y - x[3].y);
-    x[0] = make_float2(a.x + c.x, a.y + c.y);
-    x[2] = make_float2(a.x - c.x, a.y - c.y);
+    const float2 a = cadd(x[0], x[2]);
+    const float2 b = csub(x[0], x[2]);
+    const float2 c = cadd(x[1], x[3]);
+    const float2 d = csub(x[1], x[3]);
+    x[0] = cadd(a, c);
+    x[2] = csub(a, c);
     x[1] = make_float2(b.x + d.y, b.y - d.x);   // b - i d
     x[3] = make_float2(b.x - d.y, b.y + d.x);   // b + i d
 }
@@ -95,15 +130,16 @@ __device__ __forceinline__ void butterfly<5>(float2 (&x)[5])
 {
     const float c1 = 0.30901699437494742f, c2 = -0.80901699437494742f;   // cos(2pi/5), cos(4pi/5)
     const float s1 = 0.95105651629515357f, s2 = 0.58778525229247313f;    // sin(2pi/5), sin(4pi/5)
-    const float2 t1 = make_float2(x[1].x + x[4].x, x[1].y + x[4].y);
-    const float2 t2 = make_float2(x[2].x + x[3].x, x[2].y + x[3].y);
-    const float2 t3 = make_float2(x[1].x - x[4].x, x[1].y - x[4].y);
-    const float2 t4 = make_float2(x[2].x - x[3].x, x[2].y - x[3].y);
-    const float2 m1 = make_float2(x[0].x + c1 * t1.x + c2 * t2.x, x[0].y + c1 * t1.y + c2 * t2.y);
-    const float2 m2 = make_float2(x[0].x + c2 * t1.x + c1 * t2.x, x[0].y + c2 * t1.y + c1 * t2.y);
-    const float2 n1 = make_float2(s1 * t3.x + s2 * t4.x, s1 * t3.y + s2 * t4.y);
-    const float2 n2 = make_float2(s2 * t3.x - s1 * t4.x, s2 * t3.y - s1 * t4.y);
-    x[0] = make_float2(x[0].x + t1.x + t2.x, x[0].y + t1.y + t2.y);
+    const float2 t1 = cadd(x[1], x[4]);
+    const float2 t2 = cadd(x[2], x[3]);
+    const float2 t3 = csub(x[1], x[4]);
+    const float2 t4 = csub(x[2], x[3]);
+    const float2 C1 = make_float2(c1, c1), C2 = make_float2(c2, c2), S1 = make_float2(s1, s1), S2 = make_float2(s2, s2);
+    const float2 m1 = fma2(C2, t2, fma2(C1, t1, x[0]));
+    const float2 m2 = fma2(C1, t2, fma2(C2, t1, x[0]));
+    const float2 n1 = fma2(S2, t4, make_float2(s1 * t3.x, s1 * t3.y));
+    const float2 n2 = fma2(make_float2(-s1, -s1), t4, make_float2(s2 * t3.x, s2 * t3.y));
+    x[0] = cadd(cadd(x[0], t1), t2);
     x[1] = make_float2(m1.x + n1.y, m1.y - n1.x);   // m1 - i n1
     x[4] = make_float2(m1.x - n1.y, m1.y + n1.x);   // m1 + i n1
     x[2] = make_float2(m2.x + n2.y, m2.y - n2.x);

@@ -74,8 +74,10 @@ __device__ __forceinline__ void fft_dif(float2 (&x)[M])
 #pragma unroll
             for (int i = 0; i < len / 2; ++i) {
                 const float2 a = x[blk + i], b = x[blk + i + len / 2];
-                x[blk + i] = make_float2(a.x + b.x, a.y + b.y);
-                x[blk + i + len / 2] = mul_w32(make_float2(a.x - b.x, a.y - b.y), i * (32 / len));
+                const int m = i * (32 / len);
+                x[blk + i] = cadd(a, b);
+                // m = 8 (times -i) swaps the halves: scalar subtractions write them where they are wanted
+                x[blk + i + len / 2] = (m == 8) ? make_float2(a.y - b.y, b.x - a.x) : mul_w32(csub(a, b), m);
             }
         }
     }
@@ -94,6 +96,7 @@ struct FPow2Config {
     static constexpr int R2 = N / R1;
     static constexpr int W = N / PTS;             // warps per CTA
     static constexpr int THREADS = 32 * W;
+    static constexpr int MIN_CTAS = (N == 128) ? 4 : 0;   // N = 128: hold the kernel to 64 registers (four CTAs per SM); 0 = no constraint
     static constexpr int RPT = PTS / R1;          // residues per thread in pass 1
     static constexpr int KPT = PTS / R2;          // k1 values per thread in pass 2
     static constexpr int ROW_WORDS = N / 2 + 1;   // padded raw row: bank(row, word) = row + word (mod 32)
@@ -111,7 +114,7 @@ struct FPow2Config {
 // FULL : K == N (every bin is kept; no range checks)          SCALE : multiply by sw[p] (averaging weights)
 // DELAY: fractional-delay / phase gain per (input, frame) (PAPER.md 2.5.1 L266-272)
 template <int N, int R1, int PTS, bool FULL, bool SCALE, bool DELAY = false>
-__global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2_kernel(const FParams P)
+__global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<N, R1, PTS>::MIN_CTAS) f_stage_pow2_kernel(const FParams P)
 {
     using C = FPow2Config<N, R1, PTS>;
     constexpr int R2 = C::R2;
@@ -172,6 +175,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
     // int8 -> fp32 with the F-stage scale s = 2^-sh folded in (exact): byte b -> ((b ^ 0x80) + 2^23 - (2^23 + 128)) * s
     const float s = P.in_scale;
     const float bias = -8388736.0f * s;
+    const float2 ss = make_float2(s, s), bb = make_float2(bias, bias);
     const uint32_t *rrow = raw + lane * C::ROW_WORDS + (C::RPT == 2 ? w : (w >> 1));
     float2 *ex_w = ex + (w * C::RPT) * 32 + lane;                     // + (k1 * R2 + e) * 32
     const float2 *ex_r = ex + (w * C::KPT) * R2 * 32 + lane;          // + (e * R2 + r) * 32
@@ -196,15 +200,12 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS) f_stage_pow2
                 if (C::RPT == 2) {
                     // samples q = 2w + R2 j and q + 1 share one 32-bit word
                     const uint32_t word = rrow[(R2 / 2) * j] ^ 0x80808080u;
-                    x[0][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), s, bias),
-                                          fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441)), s, bias));
-                    x[C::RPT - 1][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7442)), s, bias),
-                                                   fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7443)), s, bias));
+                    x[0][j] = fma2(make_float2(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), __uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441))), ss, bb);
+                    x[C::RPT - 1][j] = fma2(make_float2(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7442)), __uint_as_float(__byte_perm(word, 0x4B000000u, 0x7443))), ss, bb);
                 } else {
                     uint32_t word = rrow[(R2 / 2) * j] ^ 0x80808080u;
                     if (w & 1) word >>= 16;
-                    x[0][j] = make_float2(fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), s, bias),
-                                          fmaf(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441)), s, bias));
+                    x[0][j] = fma2(make_float2(__uint_as_float(__byte_perm(word, 0x4B000000u, 0x7440)), __uint_as_float(__byte_perm(word, 0x4B000000u, 0x7441))), ss, bb);
                 }
             }
 #pragma unroll
