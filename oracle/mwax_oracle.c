@@ -13,6 +13,8 @@
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"): brute-force DFT, numpy.fft on special cases, tone ->
  * bin/position, Parseval, Hermitian symmetry, phase closure, additivity, weight-table invariants stated in
  * the paper (L290-306), the K=8,F=2 worked table, Fig.14 data rates, common-signal correlation coefficient.
+ * Steps 3b/3c/7/8 (delay, de-ripple gains, MWAX_ORDER, occupancy weights): shift theorem vs numpy.roll, numpy-scaled
+ * channels and a numpy.fft-made passband ripple flattened by its inverse, Fig. 8 row order, numpy counts.
  * "parity unpinned" items (no instrument data in the container): which operand is conjugated (reading Q2),
  * absolute scale of the DFT and sum-vs-mean over time (Q1, Q5) — DESIGN.md §3.
  */
@@ -236,6 +238,23 @@ int mwax_oracle_apply_delays(int n_sel, const int *sel, int N, int K, int T, int
     return ORACLE_OK;
 }
 
+/* Step 3c ("PFB de-ripple magnitude"; PAPER.md 4.2 L561-567): the gain table of the
+ * fractional-delay stage "could be combined with a spectral magnitude response that represents the inverse of the
+ * receiver PFB's passband response.  As the delays are applied, the spectral samples will then simultaneously be
+ * magnitude-adjusted to provide a flattened overall frequency response."  One real, non-negative magnitude per kept
+ * fine channel, the same for every signal path (one passband response; per-receiver-type tables are "not currently
+ * supported", L571) and every frame (reading Q23):
+ *     Y[p][t][s] *= gain[p],   p = channel position of step 3 (ascending signed frequency, DC at floor(K/2)). */
+int mwax_oracle_apply_channel_gains(int n_sel, int K, int T, const double *gain, double *Y_ri)
+{
+    if (n_sel < 1 || K < 1 || T < 1 || !gain || !Y_ri) return ORACLE_ERR_ARG;
+    cplx *Y = (cplx *)Y_ri;
+    for (int p = 0; p < K; ++p)
+        for (int t = 0; t < T; ++t)
+            for (int s = 0; s < n_sel; ++s) Y[((size_t)p * T + t) * n_sel + s] *= gain[p];
+    return ORACLE_OK;
+}
+
 /* Step 4: R[p][a(a+1)/2 + b] = sum_{t<T} Y_a[p][t] * conj(Y_b[p][t]) for all a >= b (autos included):
  * "cross-multiply every input pair", summed (not averaged) over the integration
  * (L280; reading Q5).  Direct per-pair multiply-accumulate.  Reading Q2: the SECOND index is conjugated. */
@@ -295,10 +314,10 @@ int mwax_oracle_average(int n_sel, int K, int F, int mode, const double *R_ri, d
 
 /* Whole float path for one dump and a selection of inputs (steps 1-6 in order).
  * vis: [C][n_sel(n_sel+1)/2][re,im] float64; pair (a,b), a >= b, refers to inputs sel[a], sel[b].
- * The _delay form inserts step 3b between steps 3 and 4. */
-int mwax_oracle_fx_delay(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,
-                         const int8_t *volt, int64_t row_pitch, const double *delay, const double *phase,
-                         int64_t row_stride, double *vis_ri)
+ * The _delay form inserts step 3b between steps 3 and 4, the _gain form steps 3b and 3c. */
+int mwax_oracle_fx_gain(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,
+                        const int8_t *volt, int64_t row_pitch, const double *delay, const double *phase,
+                        int64_t row_stride, const double *gain, double *vis_ri)
 {
     if (n_sel < 1 || K < 1 || F < 1 || K % F != 0 || T < 1) return ORACLE_ERR_ARG;
     const size_t B = (size_t)n_sel * (n_sel + 1) / 2;
@@ -308,11 +327,19 @@ int mwax_oracle_fx_delay(int n_sel, const int *sel, int N, int K, int T, int F, 
     int rc = mwax_oracle_spectra(n_sel, sel, N, K, T, dump, volt, row_pitch, Y);
     if (rc == ORACLE_OK && (delay || phase))
         rc = mwax_oracle_apply_delays(n_sel, sel, N, K, T, dump, delay, phase, row_stride, Y);
+    if (rc == ORACLE_OK && gain) rc = mwax_oracle_apply_channel_gains(n_sel, K, T, gain, Y);
     if (rc == ORACLE_OK) rc = mwax_oracle_correlate(n_sel, K, T, Y, R);
     if (rc == ORACLE_OK) rc = mwax_oracle_average(n_sel, K, F, mode, R, vis_ri);
     free(Y);
     free(R);
     return rc;
+}
+
+int mwax_oracle_fx_delay(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,
+                         const int8_t *volt, int64_t row_pitch, const double *delay, const double *phase,
+                         int64_t row_stride, double *vis_ri)
+{
+    return mwax_oracle_fx_gain(n_sel, sel, N, K, T, F, mode, dump, volt, row_pitch, delay, phase, row_stride, NULL, vis_ri);
 }
 
 int mwax_oracle_fx(int n_sel, const int *sel, int N, int K, int T, int F, int mode, int dump,

@@ -51,6 +51,9 @@ def _load():
                                                  dp, dp, ctypes.c_int64, dp]
         lib.mwax_oracle_fx_delay.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                              ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp, dp, ctypes.c_int64, dp]
+        lib.mwax_oracle_apply_channel_gains.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp]
+        lib.mwax_oracle_fx_gain.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                            ctypes.c_int, ctypes.c_int, i8p, ctypes.c_int64, dp, dp, ctypes.c_int64, dp, dp]
         lib.mwax_oracle_mwax_order.argtypes = [ctypes.c_int, ctypes.c_int, dp, dp, dp]
         lib.mwax_oracle_occupancy.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.POINTER(ctypes.c_uint8), ctypes.c_int,
                                               ctypes.c_int, dp, dp]
@@ -152,10 +155,21 @@ def apply_delays(Y: np.ndarray, N: int, delay=None, phase=None, dump: int = 0, s
     return Y
 
 
+def apply_channel_gains(Y: np.ndarray, gain) -> np.ndarray:
+    """Step 3c: Y complex128 [K][T][n_sel] times the real per-channel magnitude gain[K] (PFB de-ripple)."""
+    Y = np.array(Y, dtype=np.complex128, order="C")
+    K, T, n_sel = Y.shape
+    g = np.ascontiguousarray(gain, dtype=np.float64)
+    assert g.shape == (K,)
+    _check(_load().mwax_oracle_apply_channel_gains(n_sel, K, T, _dp(g), _dp(Y.view(np.float64))), "apply_channel_gains")
+    return Y
+
+
 def fx(volt: np.ndarray, N: int, K: int, T: int, F: int, mode: int = AVG_CENTRE_SYMMETRIC, dump: int = 0,
-       sel=None, delay=None, phase=None) -> np.ndarray:
+       sel=None, delay=None, phase=None, gain=None) -> np.ndarray:
     """Whole float path, one dump: int8 [n][samples][2] -> V complex128 [K/F][n_sel(n_sel+1)/2].
-    delay / phase: optional [n][frames] tables of the fractional-delay correction (step 3b)."""
+    delay / phase: optional [n][frames] tables of the fractional-delay correction (step 3b);
+    gain: optional [K] per-channel magnitudes (step 3c)."""
     assert volt.dtype == np.int8 and volt.ndim == 3 and volt.shape[2] == 2 and volt.flags.c_contiguous
     assert volt.shape[1] >= (dump + 1) * T * N
     s, sp = _sel(sel, volt.shape[0])
@@ -166,9 +180,14 @@ def fx(volt: np.ndarray, N: int, K: int, T: int, F: int, mode: int = AVG_CENTRE_
     if d is not None or ph is not None:
         stride = (d if d is not None else ph).shape[1]
         assert stride >= (dump + 1) * T and (d is None or ph is None or d.shape == ph.shape)
-    _check(_load().mwax_oracle_fx_delay(s.size, sp, N, K, T, F, mode, dump,
-                                        volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), volt.shape[1],
-                                        dpp, php, stride, _dp(V.view(np.float64))), "fx")
+    g = None
+    if gain is not None:
+        g = np.ascontiguousarray(gain, dtype=np.float64)
+        assert g.shape == (K,)
+    _check(_load().mwax_oracle_fx_gain(s.size, sp, N, K, T, F, mode, dump,
+                                       volt.ctypes.data_as(ctypes.POINTER(ctypes.c_int8)), volt.shape[1],
+                                       dpp, php, stride, _dp(g) if g is not None else None,
+                                       _dp(V.view(np.float64))), "fx")
     return V
 
 

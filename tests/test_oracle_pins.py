@@ -508,3 +508,68 @@ def test_occupancy_normalisation_restores_visibility_magnitudes():
     ratio_norm = abs(Mn[r01, 0, 2]) / abs(full[r01, 0, 2])
     assert abs(ratio_raw - 0.75) < 0.05 and abs(ratio_norm - 1.0) < 0.05
     assert np.array_equal(Mn[r01, :, 0], M[r01, :, 0])                 # weight 1.0: untouched
+
+
+# ------------------------------------------------------------------ step 3c: per-channel magnitude gains (PFB de-ripple, PAPER.md 4.2)
+def test_channel_gains_scale_each_fine_channel_by_gain_squared():
+    """F = 1: V'[p] = gain[p]^2 V[p] (both operands of every product carry the gain); the expected values are the
+    UNGAINED oracle output scaled in numpy.  An un-squared gain, a gain on one operand only, or a gain indexed in FFT
+    order instead of centre order all fail here."""
+    n, N, K, T = 3, 16, 12, 5
+    volt = rng.integers(-100, 100, size=(n, T * N, 2)).astype(np.int8)
+    gain = 0.5 + rng.random(K)
+    V0 = oracle.fx(volt, N, K, T, 1)
+    V1 = oracle.fx(volt, N, K, T, 1, gain=gain)
+    np.testing.assert_allclose(V1, V0 * (gain ** 2)[:, None], rtol=1e-12, atol=1e-9)
+    np.testing.assert_array_equal(oracle.fx(volt, N, K, T, 1, gain=np.ones(K)), V0)
+
+
+def test_channel_gains_tone_power_follows_its_own_channel():
+    """A tone on signed bin u0 sits at position u0 + K/2: only THAT entry of the gain table changes its power."""
+    N = K = 32
+    T, u0, a = 4, -7, 20.0
+    m = np.arange(T * N)
+    x = a * np.exp(2j * np.pi * u0 * m / N)
+    volt = _volt_from_complex(x[None, :])
+    base = oracle.fx(volt, N, K, T, 1)[:, 0].real
+    for p_changed in (u0 + K // 2, (u0 % N)):                  # the right index, and the FFT-order index (wrong one)
+        gain = np.ones(K)
+        gain[p_changed] = 3.0
+        got = oracle.fx(volt, N, K, T, 1, gain=gain)[:, 0].real
+        ratio = got[u0 + K // 2] / base[u0 + K // 2]
+        assert np.isclose(ratio, 9.0 if p_changed == u0 + K // 2 else 1.0, rtol=1e-9)
+
+
+def test_channel_gains_with_averaging_equal_numpy_scaled_fine_channels():
+    """F > 1: the gained dump equals the paper's weighted mean (weights() is pinned by P6-P8 and the golden table) of
+    the numpy-scaled fine-channel products."""
+    n, N, K, T, F = 2, 40, 40, 3, 4
+    volt = rng.integers(-60, 60, size=(n, T * N, 2)).astype(np.int8)
+    gain = 0.8 + 0.4 * rng.random(K)
+    R = oracle.correlate(oracle.spectra(volt, N, K, T))        # [K][B]
+    W = oracle.weights(K, F)                                   # [C][K]
+    expect = W @ (R * (gain ** 2)[:, None])
+    expect[:, [0, 2]] = expect[:, [0, 2]].real                 # autos (baselines 0 and 2 of n = 2)
+    np.testing.assert_allclose(oracle.fx(volt, N, K, T, F, gain=gain), expect, rtol=1e-11, atol=1e-7)
+
+
+def test_deripple_flattens_a_known_passband_ripple():
+    """PAPER.md 4.2 L567: gains equal to the inverse of the passband magnitude response give 'a flattened overall
+    frequency response'.  White noise is given a known ripple H(u) per frame with numpy.fft (a library routine, circular
+    filtering), quantised to int8, and correlated with gain = 1 / H: the auto spectrum must come out flat, and without
+    the gains it must follow H^2."""
+    N = K = 64
+    T, sigma = 600, 20.0
+    u = np.arange(K) - K // 2                                  # signed bin of position p
+    H_pos = 1.0 + 0.3 * np.cos(2 * np.pi * u / K) - 0.15 * np.sin(6 * np.pi * u / K)   # deliberately not symmetric in u
+    H_fft = np.fft.ifftshift(H_pos)                            # FFT order (bin k = u mod N)
+    g = sigma * (rng.standard_normal((T, N)) + 1j * rng.standard_normal((T, N)))
+    x = np.fft.ifft(np.fft.fft(g, axis=1) * H_fft[None, :], axis=1).reshape(1, T * N)
+    volt = _volt_from_complex(x)
+    raw = oracle.fx(volt, N, K, T, 1)[:, 0].real
+    flat = oracle.fx(volt, N, K, T, 1, gain=1.0 / H_pos)[:, 0].real
+    level = 2 * sigma ** 2 * N * T                             # E|X[k]|^2 summed over T spectra
+    # chi-square scatter of a T-spectrum sum: 1/sqrt(T) = 4 %; int8 rounding adds 1/6 to 800 (0.02 %)
+    assert np.all(np.abs(flat / level - 1.0) < 5 / np.sqrt(T))
+    assert np.all(np.abs(raw / (level * H_pos ** 2) - 1.0) < 5 / np.sqrt(T))
+    assert np.std(raw / level) > 5 * np.std(flat / level)      # the ripple was really there, and is gone
