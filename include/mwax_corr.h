@@ -89,6 +89,17 @@ int mwax_corr_set_option(mwax_corr_t *h, int key, int value);
 int mwax_corr_set_delays(mwax_corr_t *h, const float *d_delay, const float *d_phase, size_t row_stride,
                          size_t coarse_stride);
 
+/* Per-channel magnitude gains — "PFB de-ripple" (§4.2): the gain table of
+ * the delay stage "could be combined with a spectral magnitude response that represents the inverse of the receiver
+ * PFB's passband response", so that the spectra are "magnitude-adjusted to provide a flattened overall frequency
+ * response".  Every spectral sample of kept channel position p (ascending signed frequency, DC at n_keep/2) of every
+ * signal path and frame is multiplied by gain[p] before cross-correlation, so fine channel p's products carry
+ * gain[p]^2 into the average (reading Q23).  Folded into the F kernels' per-channel factor: no extra pass.
+ *   gain  HOST float [n_keep], each in [0, 4] (fp16 headroom), copied by the call; NULL switches the gains off.
+ * Synchronous (rebuilds the small device tables); call between, not during, process calls.
+ * MWAX_ERR_INVALID_ARG for a value outside [0, 4] or NaN. */
+int mwax_corr_set_channel_gains(mwax_corr_t *h, const float *gain);
+
 /* One integration:
  *   d_volt  in : int8 [n_inputs][T*N][re,im] — row i is signal path i's contiguous sample stream
  *                (PAPER.md L260), row pitch exactly T*N samples; two's-complement, -128 accepted.

@@ -74,6 +74,7 @@ def lib() -> ctypes.CDLL:
         L.mwax_corr_f_stage.argtypes = [vp, vp, sz, vp]
         L.mwax_corr_set_delays.argtypes = [vp, vp, vp, sz, sz]
         L.mwax_corr_set_workspace.argtypes = [vp, vp, sz]
+        L.mwax_corr_set_channel_gains.argtypes = [vp, vp]
         L.mwax_corr_to_mwax_order.argtypes = [vp, vp, vp, vp, vp]
         L.mwax_corr_to_mwax_order_weighted.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
         L.mwax_corr_mwax_order_bytes.restype = sz
@@ -202,6 +203,16 @@ class MwaxCorr:
         _check(lib().mwax_corr_set_delays(self._h, delay.data_ptr() if delay is not None else None,
                                           phase.data_ptr() if phase is not None else None, row_stride,
                                           row_stride * self.n_inputs), "mwax_corr_set_delays", self._h)
+
+    def set_channel_gains(self, gain):
+        """gain: float32 host array-like [n_keep] of per-channel magnitudes in [0, 4] (PFB de-ripple, PAPER.md 4.2);
+        None switches them off.  The library copies the values."""
+        if gain is None:
+            _check(lib().mwax_corr_set_channel_gains(self._h, None), "mwax_corr_set_channel_gains", self._h)
+            return
+        g = torch.as_tensor(gain, dtype=torch.float32, device="cpu").contiguous()
+        assert g.numel() == self.n_keep
+        _check(lib().mwax_corr_set_channel_gains(self._h, g.data_ptr()), "mwax_corr_set_channel_gains", self._h)
 
     def to_mwax_order(self, vis: torch.Tensor, out: torch.Tensor | None = None, weights: torch.Tensor | None = None,
                       stream=None, flags: torch.Tensor | None = None, normalise: bool = False):

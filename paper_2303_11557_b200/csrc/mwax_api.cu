@@ -288,6 +288,7 @@ struct mwax_corr {
     float *d_out;
     size_t out_bytes;
     const float *d_delay, *d_phase;        // caller-owned delay / phase tables (mwax_corr_set_delays), NULL = off
+    std::vector<float> gains;              // per-channel magnitude gains (mwax_corr_set_channel_gains); empty = off
     size_t d_row_stride, d_coarse_stride;
     cudaStream_t s_in, s_out;              // copy streams of process_host
     cudaEvent_t ev_start, ev_copied;
@@ -373,6 +374,14 @@ static int build_tables(mwax_corr *h)
             code[k % 400] |= cd << (2 * (k / 400));
         }
         if ((rc = upload(&h->d_swcode, code)) != MWAX_OK) return rc;
+    }
+    if (!h->gains.empty()) {
+        // PFB de-ripple magnitudes (PAPER.md 4.2): folded into the same per-position factor; the 2-bit codes above no
+        // longer describe it, so the N = 6400 kernel is launched in its table-reading (non-FULL) form while gains are set
+        for (int p = 0; p < K; ++p) sw[p] *= h->gains[p];
+        h->chan_scale = 1;
+        cudaFree(h->d_sw); h->d_sw = nullptr;
+        if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
     }
     if ((rc = upload(&h->d_tap_start, tap)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_scale, scale)) != MWAX_OK) return rc;
@@ -490,6 +499,21 @@ int mwax_corr_set_option(mwax_corr_t *h, int key, int value)
     return MWAX_ERR_INVALID_ARG;
 }
 
+int mwax_corr_set_channel_gains(mwax_corr_t *h, const float *gain)
+{
+    if (!h) return MWAX_ERR_NULL;
+    if (!gain) {
+        if (h->gains.empty()) return MWAX_OK;
+        h->gains.clear();
+        return build_tables(h);
+    }
+    // |Y| <= 127 sqrt(2) N s gain with s ~ 1/sqrt(N) must stay inside fp16: gain <= 4 leaves a factor > 1.1 at N = 6400
+    for (int p = 0; p < h->K; ++p)
+        if (!(gain[p] >= 0.0f && gain[p] <= 4.0f)) return MWAX_ERR_INVALID_ARG;
+    h->gains.assign(gain, gain + h->K);
+    return build_tables(h);
+}
+
 static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, int frame0, int coarse, void *stream)
 {
     if (!h || !d_volt) return MWAX_ERR_NULL;
@@ -510,7 +534,7 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
     cudaStream_t st = (cudaStream_t)stream;
     const int f_kind = fp.vec_ok ? h->f_kind : 0;          // misaligned rows: generic kernel (scalar loads)
     if (f_kind == 6400) {
-        const bool full = (h->K == h->N), scale = (h->chan_scale != 0) || !full;
+        const bool full = (h->K == h->N) && h->gains.empty(), scale = (h->chan_scale != 0) || !full;
         int rc = h->f_p3 == 8 ? launch_f_6400p3<8>(fp, full, scale, delay, st) : h->f_p3 == 4 ? launch_f_6400p3<4>(fp, full, scale, delay, st)
                                                                         : launch_f_6400p3<2>(fp, full, scale, delay, st);
         if (rc != MWAX_OK) return rc;

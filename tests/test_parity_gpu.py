@@ -310,6 +310,59 @@ def test_delay_phase_correction_elementwise(n, N, K, T, F):
     h.destroy()
 
 
+# SURVEY.md 8(f) NEXT #1, second half: per-channel magnitude gains ("PFB de-ripple", PAPER.md 4.2 L561-567) folded
+# into the F kernels' per-channel factor
+@pytest.mark.parametrize("n,N,K,T,F,mode", [
+    (16, 64, 64, 12, 1, 0),        # register kernel, F = 1 (the unscaled variant becomes the scaled one)
+    (20, 128, 96, 9, 4, 0),        # keep < fft, centre-symmetric weights times gains
+    (33, 256, 256, 5, 2, 0),       # shared edge taps (sqrt(1/2) times gain)
+    (12, 100, 100, 7, 5, 1),       # generic Stockham kernel, BLOCK mode
+    (10, 6400, 6400, 3, 50, 0),    # the paper's mode: the three-pass kernel leaves its 2-bit weight codes for the table
+    (6, 6400, 5000, 2, 50, 0),     # keep < fft at N = 6400
+])
+def test_channel_gains_elementwise(n, N, K, T, F, mode):
+    rng = np.random.default_rng(300 + n + N)
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.3, tones=[synth.Tone(min(3, K // 2 - 1), 6.0, 1)], seed=3000 + n + N)
+    volt = synth.gauss_voltages(spec)
+    u = np.arange(K) - K // 2
+    gain = (1.0 + 0.25 * np.cos(2 * np.pi * u / K) + 0.1 * rng.standard_normal(K)).astype(np.float32)   # a ripple's inverse
+    ref = oracle.fx(volt, N, K, T, F, mode=mode, gain=gain.astype(np.float64))
+    plain = oracle.fx(volt, N, K, T, F, mode=mode)
+    h = corr.MwaxCorr(n, N, K, T, F, avg_mode=mode)
+    v = torch.from_numpy(volt).cuda()
+    out = h.new_output()
+    h.set_channel_gains(gain)
+    h.process(v, out[0, 0])
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy()[0, 0])
+    assert _norm_err(got, ref, n) <= TOL
+    assert _norm_err(got, plain, n) > 0.05, "the gains must change the visibilities"
+    # together with the delay / phase correction (the paper's combined look-up table)
+    delay = rng.uniform(-0.5, 0.5, size=(n, T)).astype(np.float32)
+    phase = rng.uniform(-np.pi, np.pi, size=(n, T)).astype(np.float32)
+    h.set_delays(torch.from_numpy(delay).cuda(), torch.from_numpy(phase).cuda())
+    h.process(v, out[0, 0])
+    torch.cuda.synchronize()
+    both = oracle.fx(volt, N, K, T, F, mode=mode, delay=delay.astype(np.float64), phase=phase.astype(np.float64),
+                     gain=gain.astype(np.float64))
+    assert _norm_err(_complex(out.cpu().numpy()[0, 0]), both, n) <= TOL
+    # off again: back to the plain path (and, at N = 6400, to the 2-bit weight codes)
+    h.set_delays(None, None)
+    h.set_channel_gains(None)
+    h.process(v, out[0, 0])
+    torch.cuda.synchronize()
+    assert _norm_err(_complex(out.cpu().numpy()[0, 0]), plain, n) <= TOL
+    # out-of-range gains are refused
+    bad = gain.copy()
+    bad[K // 3] = 5.0
+    with pytest.raises(corr.MwaxError):
+        h.set_channel_gains(bad)
+    bad[K // 3] = np.nan
+    with pytest.raises(corr.MwaxError):
+        h.set_channel_gains(bad)
+    h.destroy()
+
+
 def test_delay_tables_follow_dumps_and_coarse_channels():
     n, N, T, D, NC = 8, 64, 6, 2, 2
     rng = np.random.default_rng(3)
