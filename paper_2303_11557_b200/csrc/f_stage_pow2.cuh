@@ -103,7 +103,8 @@ struct FPow2Config {
     static constexpr int RAW_WORDS = 32 * ROW_WORDS;
     static constexpr int TW_WORDS = 2 * N;        // inter-pass twiddles [r][k1] float2
     static constexpr int EX_OFF_WORDS = ((RAW_WORDS + TW_WORDS + 3) / 4) * 4;
-    static constexpr int SMEM_BYTES = EX_OFF_WORDS * 4 + N * 32 * 8;
+    static constexpr int SW_OFF_WORDS = EX_OFF_WORDS + N * 32 * 2;    // per-position factors sqrt(w_p) [K <= N] (SCALE variants)
+    static constexpr int SMEM_BYTES = SW_OFF_WORDS * 4 + N * 4;
     static constexpr int VPT = (32 * (N / 8)) / THREADS;   // 16-byte raw vectors per thread per frame
     static_assert(RPT >= 1 && KPT >= 1 && (RPT == 1 || RPT == 2), "unsupported split");
     static_assert(R1 * R2 == N && W * RPT == R2 && W * KPT == R1, "bad factorisation");
@@ -122,6 +123,8 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
     uint32_t *raw = fsm;                                              // [32 rows][ROW_WORDS]
     float2 *twp = reinterpret_cast<float2 *>(fsm + C::RAW_WORDS + (C::RAW_WORDS & 1));   // [R2][R1] W_N^{r k1}
     float2 *ex = reinterpret_cast<float2 *>(fsm + C::EX_OFF_WORDS);  // [k1][r][lane]
+    float *swt = reinterpret_cast<float *>(fsm + C::SW_OFF_WORDS);   // sqrt(w_p): the channel of a store is warp uniform, so
+                                                                      // these are broadcast reads (was a global load per bin)
 
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i0 = blockIdx.x * 32;
@@ -133,6 +136,8 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
         const int r = e / R1, k1 = e % R1;
         twp[e] = __ldg(&P.tw[r * k1]);
     }
+    if (SCALE)
+        for (int e = threadIdx.x; e < P.K; e += C::THREADS) swt[e] = __ldg(&P.sw[e]);
     constexpr int VPR = N / 8;                                        // 16-byte vectors per row
     const int8_t *src[C::VPT];
     uint32_t *rdst[C::VPT];
@@ -240,7 +245,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                 // k < N/2  <=>  k2 < R2/2:  p = k + N/2, else p = k - N/2
                 __half2 *yp = ybase + ((size_t)(k1 + N / 2) * P.T + t) * P.pitch2;
                 __half2 *yn = ybase + ((size_t)k1 * P.T + t) * P.pitch2;
-                const float *swp = P.sw + k1;
+                const float *swp = swt + k1;
                 if (iok) {
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) {
@@ -248,7 +253,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                         if (DELAY) v = apply_delay_gain(v, gn, k1 + ((k2 < R2 / 2) ? R1 * k2 : R1 * k2 - N));
                         const int pk = (k2 < R2 / 2) ? (N / 2 + R1 * k2) : (R1 * k2 - N / 2);   // p - k1
                         if (SCALE) {
-                            const float f = __ldg(swp + pk);
+                            const float f = swp[pk];
                             v.x *= f;
                             v.y *= f;
                         }
@@ -267,7 +272,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                     float2 v = y[bitrev(k2, ilog2(R2))];
                     if (DELAY) v = apply_delay_gain(v, gn, u);
                     if (SCALE) {
-                        const float f = __ldg(&P.sw[p]);                     // sqrt(w_p): shared edge / DC exclusion
+                        const float f = swt[p];                              // sqrt(w_p): shared edge / DC exclusion
                         v.x *= f;
                         v.y *= f;
                     }
