@@ -28,6 +28,7 @@
 #include <cstdint>
 #include "f_stage.cuh"
 #include "f_stage_pow2.cuh"
+#include "ptx.cuh"
 
 namespace mwax {
 
@@ -143,6 +144,19 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
     }
     __syncthreads();
 
+    // Q = 2: the partner's fp16 rows are PUSHED into this CTA by bulk copies (one per k1: its 20 slots are contiguous, 2560 bytes;
+    // completion counted on `rx_bar`) into the slots of input 1, free once pass 3 has read them; the
+    // store phase then reads local shared memory only.  Pulling the rows with ld.shared::cluster inside the store loop
+    // left every store waiting on a remote load: 37 % of the kernel's stall samples (profiles/r1_ncu_full.md).
+    constexpr bool PUSH = (Q == 2);
+    constexpr int RX_OFF = C::SG;                                    // float2 index of the receive area (16-byte aligned)
+    __shared__ __align__(8) unsigned long long rx_bar;
+    const uint32_t rx_bar_a = ptx::smem_u32(&rx_bar);
+    uint32_t rx_phase = 0;
+    if (PUSH && threadIdx.x == 0) {
+        ptx::mbar_init(rx_bar_a, 1);
+        ptx::fence_mbar_init();
+    }
     const uint32_t rank = cluster_ctarank();
     const int g = threadIdx.x & 3, j = threadIdx.x >> 2;             // j in [0,160)
     const int hi = j >> 3, lo = j & 7;                               // hi = warp index (warp-uniform), in [0,20)
@@ -274,8 +288,25 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
                 ((k3 < 8) ? s_lo : s_hi)[(k3 & 7) * 4] = *reinterpret_cast<const uint32_t *>(&hv);
             }
         }
+        if (PUSH) {
+            ptx::fence_proxy_async();                                // the staged rows will be read by bulk copies
+            if (threadIdx.x == 0) ptx::mbar_arrive_expect_tx(rx_bar_a, 400u * 128u);   // this item's incoming rows
+        }
         cluster_arrive();
         cluster_wait();                                              // every CTA of the cluster has staged its rows
+        if (PUSH) {
+            // rows of the OTHER CTA's k3 half: rank 0 sends its k3 >= 8 rows (input 3's slots), rank 1 its k3 < 8 rows
+            // the 20 slots (k2) of one k1 are contiguous: 20 copies of 2560 bytes
+            if (threadIdx.x < 20) {
+                const int slot = threadIdx.x * C::S1;
+                const uint32_t base = (uint32_t)__cvta_generic_to_shared(esm);
+                const uint32_t src = base + (uint32_t)(((rank == 0 ? 3 * C::SG : 0) + slot) * 8);
+                const uint32_t dst = ld_dsmem_base(base + (uint32_t)((RX_OFF + slot) * 8), rank ^ 1u);
+                ptx::bulk_copy_to_cluster(dst, src, 20u * 128u, ld_dsmem_base(rx_bar_a, rank ^ 1u));
+            }
+            ptx::mbar_wait(rx_bar_a, rx_phase);                      // the partner's rows of MY k3 half have landed
+            rx_phase ^= 1u;
+        }
 
         // ---- corner-turned store: this CTA writes rows k3 in [rank 16/Q, (rank + 1) 16/Q) for all 4 Q inputs
         // Thread = (piece q = tid % Q of a row, row stream tid / Q + (640 / Q) it): 640 / Q is a multiple of 20, so k1 is
@@ -300,8 +331,14 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
                     if (b0 + e >= C::N / C::THREADS) break;
                     const int k3 = (int)rank * (16 / Q) + kl;
                     const int k2 = c / 20;
-                    const uint32_t so = (uint32_t)(((k3 < 8 ? 0 : 3 * C::SG) + k1 * C::S1 + k2 * 16) * 8 + (k3 & 7) * 16);
-                    pv[e] = ld_shared_cluster_v4(rbase + so);
+                    if (PUSH) {                                      // own piece: staged slot; partner's piece: receive area
+                        const int area = (q == (int)rank) ? (k3 < 8 ? 0 : 3 * C::SG) : RX_OFF;
+                        pv[e] = *reinterpret_cast<const uint4 *>(reinterpret_cast<const uint8_t *>(esm) +
+                                                                  (area + k1 * C::S1 + k2 * 16) * 8 + (k3 & 7) * 16);
+                    } else {
+                        const uint32_t so = (uint32_t)(((k3 < 8 ? 0 : 3 * C::SG) + k1 * C::S1 + k2 * 16) * 8 + (k3 & 7) * 16);
+                        pv[e] = ld_shared_cluster_v4(rbase + so);
+                    }
                     pk[e] = c + 400 * k3;
                     c += RSTEP;
                     if (c >= 400) { c -= 400; ++kl; }

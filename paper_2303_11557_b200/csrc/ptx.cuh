@@ -118,6 +118,15 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank)
     return r;
 }
 // arrive on an mbarrier anywhere in the cluster (address from mapa)
+// generic-proxy writes to shared memory -> visible to the async proxy (bulk copies that read them)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+// bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned) from this CTA's shared memory to the shared
+// memory of another CTA of the cluster; completion is counted in bytes on `cluster_bar`, an mbarrier of the destination CTA
+__device__ __forceinline__ void bulk_copy_to_cluster(uint32_t cluster_dst, uint32_t src, uint32_t bytes, uint32_t cluster_bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(cluster_dst), "r"(src), "r"(bytes), "r"(cluster_bar) : "memory");
+}
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar)
 {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
