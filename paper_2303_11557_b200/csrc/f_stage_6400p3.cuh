@@ -149,7 +149,9 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
     // store phase then reads local shared memory only.  Pulling the rows with ld.shared::cluster inside the store loop
     // left every store waiting on a remote load: 37 % of the kernel's stall samples (profiles/r1_ncu_full.md).
     constexpr bool PUSH = (Q == 2);
-    constexpr int RX_OFF = C::SG;                                    // float2 index of the receive area (16-byte aligned)
+    // float2 index of the receive area of CTA r: 16-byte aligned, and 64 bytes (mod 128) away from that CTA's own staged
+    // rows (input 0's slots for rank 0, input 3's for rank 1), so that the 16-byte reads of a row's two pieces never share banks
+    auto rx_off = [](uint32_t r) { return C::SG + (r ? 8 : 0); };
     __shared__ __align__(8) unsigned long long rx_bar;
     const uint32_t rx_bar_a = ptx::smem_u32(&rx_bar);
     uint32_t rx_phase = 0;
@@ -301,7 +303,7 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
                 const int slot = threadIdx.x * C::S1;
                 const uint32_t base = (uint32_t)__cvta_generic_to_shared(esm);
                 const uint32_t src = base + (uint32_t)(((rank == 0 ? 3 * C::SG : 0) + slot) * 8);
-                const uint32_t dst = ld_dsmem_base(base + (uint32_t)((RX_OFF + slot) * 8), rank ^ 1u);
+                const uint32_t dst = ld_dsmem_base(base + (uint32_t)((rx_off(rank ^ 1u) + slot) * 8), rank ^ 1u);
                 ptx::bulk_copy_to_cluster(dst, src, 20u * 128u, ld_dsmem_base(rx_bar_a, rank ^ 1u));
             }
             ptx::mbar_wait(rx_bar_a, rx_phase);                      // the partner's rows of MY k3 half have landed
@@ -332,7 +334,7 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
                     const int k3 = (int)rank * (16 / Q) + kl;
                     const int k2 = c / 20;
                     if (PUSH) {                                      // own piece: staged slot; partner's piece: receive area
-                        const int area = (q == (int)rank) ? (k3 < 8 ? 0 : 3 * C::SG) : RX_OFF;
+                        const int area = (q == (int)rank) ? (k3 < 8 ? 0 : 3 * C::SG) : rx_off(rank);
                         pv[e] = *reinterpret_cast<const uint4 *>(reinterpret_cast<const uint8_t *>(esm) +
                                                                   (area + k1 * C::S1 + k2 * 16) * 8 + (k3 & 7) * 16);
                     } else {
