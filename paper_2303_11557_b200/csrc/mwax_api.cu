@@ -215,18 +215,37 @@ int launch_x(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::
     return cudaGetLastError() == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
 }
 
-template <bool kInt8>
+// CTA pairs the device can hold at once for this kernel (GPCs with an odd SM count leave one SM unpaired); 0 on error
+template <bool kInt8, bool kEdge>
+int x_pair_capacity(int sm_count)
+{
+    using C = mwax::XPairConfig<kInt8, kEdge>;
+    auto kern = mwax::x_stage_pair_kernel<kInt8, kEdge>;
+    static int max_pairs = 0;
+    if (!max_pairs) {
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) return 0;
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        cfg.gridDim = dim3(2);
+        int n = 0;
+        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = sm_count / 2;
+        max_pairs = n < sm_count / 2 ? n : sm_count / 2;
+    }
+    return max_pairs;
+}
+
+template <bool kInt8, bool kEdge = false>
 int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::XParams &xp, int sm_count, cudaStream_t st)
 {
-    using C = mwax::XPairConfig<kInt8>;
-    auto kern = mwax::x_stage_pair_kernel<kInt8>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
-            return MWAX_ERR_CUDA;
-        attr_set = true;
-    }
-    const int n_items = xp.n_out * xp.n_tiles;
+    using C = mwax::XPairConfig<kInt8, kEdge>;
+    auto kern = mwax::x_stage_pair_kernel<kInt8, kEdge>;
+    const int max_pairs = x_pair_capacity<kInt8, kEdge>(sm_count);
+    if (max_pairs < 1) return MWAX_ERR_CUDA;
+    const int n_items = (kEdge ? xp.edge_runs : xp.n_out) * xp.n_tiles;   // units of the persistent loop
     if (n_items <= 0) return MWAX_OK;
     cudaLaunchConfig_t cfg = {};
     cudaLaunchAttribute attr[1];
@@ -234,17 +253,32 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    static int max_pairs = 0;          // pairs the device can hold at once (GPCs with an odd SM count leave one SM unpaired)
-    if (!max_pairs) {
-        cfg.gridDim = dim3(2);
-        int n = 0;
-        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = sm_count / 2;
-        max_pairs = n < sm_count / 2 ? n : sm_count / 2;
-    }
     int pairs = n_items < max_pairs ? n_items : max_pairs;   // persistent: never more pairs than run concurrently
     if (const char *e = getenv("MWAX_X_PAIRS")) { const int v = atoi(e); if (v >= 1 && v < pairs) pairs = v; }
     cfg.gridDim = dim3(2 * pairs);
     return cudaLaunchKernelEx(&cfg, kern, tmap, tmap_flat, xp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
+}
+
+// Shared-edge schedule (x_stage.cuh): how many runs of adjacent output channels per tile, or 0 when the
+// plain schedule is at least as good.  Cost model = waves of the persistent grid x taps of the longest unit: a run of L
+// channels contracts L F + 1 fine channels, the plain schedule F + 1 per channel.
+// MWAX_X_EDGE=0 never, =1 whenever the geometry allows it (tests); MWAX_X_EDGE_RUNS forces the run count.
+int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs)
+{
+    int force = -1;
+    if (const char *e = getenv("MWAX_X_EDGE")) force = atoi(e);
+    if (force == 0 || F < 2 || (F & 1) || T < 64 || pairs < 1) return 0;
+    if (const char *e = getenv("MWAX_X_EDGE_RUNS")) { const int v = atoi(e); if (v >= 1 && v <= C) return v; }
+    const long long plain = (((long long)C * n_tiles + pairs - 1) / pairs) * (F + 1);
+    long long best = -1;
+    int best_r = 0;
+    for (int r = 1; r <= C; ++r) {
+        const long long waves = ((long long)r * n_tiles + pairs - 1) / pairs;
+        const long long cost = waves * ((long long)((C + r - 1) / r) * F + 1);
+        if (best < 0 || cost < best) { best = cost; best_r = r; }
+    }
+    if (force == 1) return best_r;
+    return (best * 100 <= plain * 92) ? best_r : 0;
 }
 
 }  // namespace
@@ -277,6 +311,7 @@ struct mwax_corr {
     uint8_t *d_ptiles;  // CTA-pair kernel's tile list
     int n_ptiles, x_pair;
     int n_tiles, n_taps;
+    int edge_runs;      // shared-edge schedule of the pair kernel: runs per tile, 0 = off, -1 = not chosen yet
     __half *d_Y;
     bool y_owned;      // false after mwax_corr_set_workspace: the caller owns the memory
     size_t y_bytes;
@@ -363,6 +398,7 @@ static int build_tables(mwax_corr *h)
     std::vector<uint8_t> tiles;
     build_tiles(h->n, h->x_bn, tiles);
     h->n_tiles = (int)tiles.size() / 4;
+    h->edge_runs = -1;
     int rc;
     if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
     if (h->N == 6400 && K == 6400) {
@@ -584,9 +620,15 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
     xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = h->n_taps; xp.scale = h->d_scale;
     xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
     xp.accumulate = h->accumulate;
+    xp.edge_runs = 0;
     if (h->x_pair) {
         xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
-        int rcp = launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
+        if (h->edge_runs < 0)
+            h->edge_runs = (h->avg_mode == MWAX_AVG_CENTRE_SYMMETRIC && h->n_taps == h->F + 1)
+                               ? choose_edge_runs(h->C, h->F, h->T, h->n_ptiles, x_pair_capacity<false, true>(h->sm_count)) : 0;
+        xp.edge_runs = h->edge_runs;
+        int rcp = xp.edge_runs > 0 ? launch_x_pair<false, true>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream)
+                                   : launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
         if (rcp != MWAX_OK) note_cuda(&h->last_cuda);
         return rcp;
     }
@@ -809,6 +851,7 @@ int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, vo
     xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = 1; xp.scale = nullptr;
     xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
     xp.accumulate = 0;
+    xp.edge_runs = 0;
     if (h->x_pair) {
         xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
         rc = launch_x_pair<true>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream);

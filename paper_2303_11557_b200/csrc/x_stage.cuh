@@ -38,7 +38,17 @@ struct XParams {
     void *out;                // float2 / int2 [C][n(n+1)/2]
     long long out_chan_stride;  // n(n+1)/2
     int accumulate;             // float path: add to what `out` already holds (integration across calls) instead of overwriting
+    int edge_runs;              // pair kernel, even F, centre-symmetric averaging: > 0 = shared-edge schedule with this many
+                                // runs of adjacent output channels per tile (x_stage2.cuh); 0 = every channel on its own
 };
+
+// Shared-edge schedule: with even F the outermost fine channel of an output channel is shared, at half
+// weight, with its neighbour.  Instead of contracting it twice, a CTA pair walks a RUN of adjacent
+// output channels of one tile and keeps a running sum S per accumulator element in shared memory (thread private):
+//   INIT  edge tap below the run's first channel:        S  = e
+//   ADD   the F - 1 interior taps of channel c:          S += m
+//   OUT   the edge tap above channel c:                  V[c] = scale_c (S + e),  S = e   (it is also c + 1's lower edge)
+enum { X_EDGE_NONE = 0, X_EDGE_INIT = 1, X_EDGE_ADD = 2, X_EDGE_OUT = 3 };
 
 template <bool kInt8, int BN>
 struct XConfig {
@@ -66,9 +76,9 @@ struct XConfig {
 // i_base) and `ncc` chunks of 32 G columns (16 inputs j from j_base + 16 cc): tcgen05.ld, the 2 x 2 real -> complex
 // fold, scale, Im(auto) := 0, triangle mask, and stores staged through padded shared memory so that
 // each instruction writes 16 consecutive baselines of two rows.  `stg` = this warp's EPI_STAGE_WORDS floats.
-template <bool kInt8>
+template <bool kInt8, bool kEdge = false>
 __device__ __forceinline__ void x_epilogue_tile(const XParams &P, float *stg, uint32_t t_row, int c, int i_base, int j_base,
-                                                int ncc, float sc, int lane)
+                                                int ncc, float sc, int lane, int mode = X_EDGE_NONE, float *S = nullptr)
 {
     const int n = P.n_inputs;
 #pragma unroll 1
@@ -89,10 +99,24 @@ __device__ __forceinline__ void x_epilogue_tile(const XParams &P, float *stg, ui
                 v = __int_as_float(w);
             } else {
                 const float a = __uint_as_float(r[2 * jj]), b = __uint_as_float(other);
-                v = ((lane & 1) ? (a - b) : (a + b)) * sc;
+                float w = (lane & 1) ? (a - b) : (a + b);
+                if (kEdge) {                      // running sum over the run's taps: S[chunk][jj][lane], this warp's slice
+                    float *sp = S + (cc * 16 + jj) * 32 + lane;
+                    if (mode == X_EDGE_INIT) {
+                        *sp = w;
+                    } else if (mode == X_EDGE_ADD) {
+                        *sp += w;
+                    } else {
+                        const float sum = *sp + w;
+                        *sp = w;
+                        w = sum;
+                    }
+                }
+                v = w * sc;
             }
-            stg[(lane >> 1) * 34 + 2 * jj + (lane & 1)] = v;
+            if (!kEdge || mode == X_EDGE_OUT) stg[(lane >> 1) * 34 + 2 * jj + (lane & 1)] = v;
         }
+        if (kEdge && mode != X_EDGE_OUT) continue;   // warp-uniform: nothing to store yet
         __syncwarp();
         // coalesced store: two rows (inputs i) x 16 complex per instruction
         const int jl = lane & 15;

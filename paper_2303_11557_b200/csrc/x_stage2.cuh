@@ -18,7 +18,9 @@
 
 namespace mwax {
 
-template <bool kInt8>
+// kEdge: shared-edge schedule for even F (x_stage.cuh): 4 pipeline stages instead of 6 make room for the 64 KB of
+// running sums (128 epilogue threads x 128 folded accumulator elements)
+template <bool kInt8, bool kEdge = false>
 struct XPairConfig {
     static constexpr int BM = 128;                        // G rows per CTA (256 per pair)
     static constexpr int BN = 256;                        // G columns per pair (128 staged per CTA)
@@ -30,21 +32,24 @@ struct XPairConfig {
     static constexpr int CHUNK_BYTES = 128 * BK;
     static constexpr int A_BYTES = CHUNKS * CHUNK_BYTES;  // 16 KB
     static constexpr int STAGE_BYTES = 2 * A_BYTES;       // 32 KB per CTA
-    static constexpr int STAGES = 6;
+    static constexpr int STAGES = kEdge ? 4 : 6;
     static constexpr int ACC_STAGES = 2;
     static constexpr int TMEM_COLS = 512;
     static constexpr int EPI_STAGE_WORDS = 16 * 34;
-    static constexpr int SMEM_BYTES = 1024 + STAGES * STAGE_BYTES + 4 * EPI_STAGE_WORDS * 4 + 256;
+    static constexpr int EDGE_WORDS_PER_WARP = kEdge ? (BN / 32) * 16 * 32 : 0;   // [chunk][jj][lane] floats
+    static constexpr int EDGE_OFF = STAGES * STAGE_BYTES + 4 * EPI_STAGE_WORDS * 4 + 256;
+    static constexpr int SMEM_BYTES = 1024 + EDGE_OFF + 4 * EDGE_WORDS_PER_WARP * 4;
     static constexpr uint32_t IDESC = ptx::make_idesc(kInt8 ? 2u : 1u, kInt8 ? 1u : 0u, 256, BN);
     static constexpr int THREADS = 192;
 };
 
 // P.tiles: [n_tiles][4] = (mi, nj, 0, 0) in units of 128 inputs (256 rows / columns of G), nj <= mi
-template <bool kInt8>
+template <bool kInt8, bool kEdge = false>
 __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_constant__ CUtensorMap tmap,
                                                               const __grid_constant__ CUtensorMap tmap_flat, const XParams P)
 {
-    using C = XPairConfig<kInt8>;
+    using C = XPairConfig<kInt8, kEdge>;
+    static_assert(!(kInt8 && kEdge), "the shared-edge schedule belongs to the float path (averaging)");
     extern __shared__ uint8_t smem_raw[];
     const uint32_t smem_base = (ptx::smem_u32(smem_raw) + 1023u) & ~1023u;   // SWIZZLE_128B atoms: 1024-byte alignment
     uint8_t *smem_gen = smem_raw + (smem_base - ptx::smem_u32(smem_raw));
@@ -92,6 +97,38 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
     const int kb_per_tap = (P.T + C::BK - 1) / C::BK;
     const bool flat = (P.n_taps > 1) && (P.T >= C::BK);    // see x_stage.cuh: whole-block K loop over adjacent taps
 
+    // kEdge: the work of this pair, identical in the three roles.  Unit = (run r of adjacent output channels, tile);
+    // fn(c, tile, first tap position, taps, mode) once per accumulator (x_stage.cuh, X_EDGE_*)
+    auto for_each_edge_item = [&](auto &&fn) {
+        const int n_units = P.edge_runs * P.n_tiles;
+        for (int unit = pair; unit < n_units; unit += n_pairs) {
+            const int r = unit / P.n_tiles, tile = unit - r * P.n_tiles;
+            const int c_a = (int)(((long long)r * P.n_out) / P.edge_runs);
+            const int c_b = (int)(((long long)(r + 1) * P.n_out) / P.edge_runs);
+            fn(c_a, tile, P.tap_start[c_a], 1, (int)X_EDGE_INIT);
+            for (int c = c_a; c < c_b; ++c) {
+                int p = P.tap_start[c] + 1;
+                if (p >= P.K) p -= P.K;
+                fn(c, tile, p, P.n_taps - 2, (int)X_EDGE_ADD);
+                p = P.tap_start[c] + P.n_taps - 1;
+                if (p >= P.K) p -= P.K;
+                fn(c, tile, p, 1, (int)X_EDGE_OUT);
+            }
+        }
+    };
+    // K-loop schedule of `nt` adjacent taps from position p0 (cyclic), T >= BK: whole BK-row blocks of the flattened rows,
+    // the end of a run through the per-channel map; full(row), tail(row, chan, rows)
+    auto k_schedule = [&](int p0, int nt, auto &&full, auto &&tail) {
+        const int n1 = min(nt, P.K - p0);
+        for (int run = 0; run < 2; ++run) {
+            const int pf = run ? 0 : p0, ntr = run ? nt - n1 : n1;
+            if (ntr <= 0) continue;
+            const int rows = ntr * P.T, nfull = rows / C::BK, tl = rows - nfull * C::BK;
+            for (int q = 0; q < nfull; ++q) full(pf * P.T + q * C::BK);
+            if (tl) tail(P.T - tl, pf + ntr - 1, tl);
+        }
+    };
+
     if (warp == 0) {
         // ------------------------------------------------------------------ TMA producer (one thread in EACH CTA)
         if (lane == 0) {
@@ -118,6 +155,13 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
                 }
                 if (++s == C::STAGES) { s = 0; ph ^= 1u; }
             };
+            if (kEdge) {
+                for_each_edge_item([&](int, int tile, int p0, int nt, int) {
+                    const int mi = P.tiles[4 * tile], nj = P.tiles[4 * tile + 1];
+                    k_schedule(p0, nt, [&](int row) { load_block(&tmap_flat, mi, nj, row, 0); },
+                               [&](int row, int chan, int) { load_block(&tmap, mi, nj, row, chan); });
+                });
+            } else
             for (int item = pair; item < n_items; item += n_pairs) {
                 const int c = item / P.n_tiles;
                 const int tile = item - c * P.n_tiles;
@@ -163,6 +207,19 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
                 accumulate = 1;
                 if (++s == C::STAGES) { s = 0; ph ^= 1u; }
             };
+            if (kEdge) {
+                for_each_edge_item([&](int, int tile, int p0, int nt, int) {
+                    b_off = (P.tiles[4 * tile] == P.tiles[4 * tile + 1]) ? 0u : (uint32_t)C::A_BYTES;   // diagonal tile: B = A
+                    ptx::mbar_wait(tempty_bar(as), aph ^ 1u);
+                    ptx::tc_fence_after();
+                    d_tmem = tmem_base + (uint32_t)(as * C::BN);
+                    accumulate = 0;
+                    k_schedule(p0, nt, [&](int) { mma_block(C::BK); }, [&](int, int, int rows) { mma_block(rows); });
+                    if (ptx::elect_one()) ptx::tc_commit_pair(tfull_bar(as), 3);
+                    __syncwarp();
+                    if (++as == C::ACC_STAGES) { as = 0; aph ^= 1u; }
+                });
+            } else
             for (int item = pair; item < n_items; item += n_pairs) {
                 const int c = item / P.n_tiles;
                 const int tile = item - c * P.n_tiles;
@@ -196,6 +253,22 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
         float *stg = epi_stage + (warp - 2) * C::EPI_STAGE_WORDS;
         int as = 0;
         uint32_t aph = 0;
+        if (kEdge) {
+            float *S = reinterpret_cast<float *>(smem_gen + C::EDGE_OFF) + (warp - 2) * C::EDGE_WORDS_PER_WARP;
+            for_each_edge_item([&](int c, int tile, int, int, int mode) {
+                const int mi = P.tiles[4 * tile], nj = P.tiles[4 * tile + 1];
+                const int i_base = mi * 128 + (int)rank * 64 + q * 16;
+                const float sc = P.scale[c];
+                ptx::mbar_wait(tfull_bar(as), aph);
+                ptx::tc_fence_after();
+                const uint32_t t_row = tmem_base + ((uint32_t)(q * 32) << 16) + (uint32_t)(as * C::BN);
+                x_epilogue_tile<kInt8, kEdge>(P, stg, t_row, c, i_base, nj * 128, C::BN / 32, sc, lane, mode, S);
+                ptx::tc_fence_before();
+                __syncwarp();
+                if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(as), 0));
+                if (++as == C::ACC_STAGES) { as = 0; aph ^= 1u; }
+            });
+        } else
         for (int item = pair; item < n_items; item += n_pairs) {
             const int c = item / P.n_tiles;
             const int tile = item - c * P.n_tiles;

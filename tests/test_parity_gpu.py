@@ -533,3 +533,50 @@ def test_caller_owned_workspace_gives_the_same_result():
     with pytest.raises(corr.MwaxError):
         h.set_workspace(ws[off:off + 16])                                                      # too small
     h.destroy()
+
+
+@pytest.mark.parametrize("n,N,K,T,F,runs", [
+    (16, 64, 64, 80, 2, 5),        # 32 output channels in 5 uneven runs; channel 0's lower edge wraps to position K - 1
+    (16, 64, 64, 64, 2, 32),       # one channel per run: every unit is INIT, ADD, OUT
+    (70, 128, 96, 65, 4, 3),       # F = 4: three interior taps per channel, T one past a 64-row block, ragged inputs
+    (200, 256, 256, 70, 2, 1),     # config-5 shape cut down, several pair tiles, the whole band as one run
+    (8, 6400, 6400, 64, 50, 7),    # the paper's mode: 49 interior taps per channel
+])
+def test_shared_edge_schedule_matches_oracle(monkeypatch, n, N, K, T, F, runs):
+    """Even F, centre-symmetric averaging: the pair kernel's shared-edge schedule (each half-weight edge channel contracted
+    once per run of adjacent output channels) against the oracle, and against the plain schedule."""
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[synth.Tone(3, 6.0, 1)], seed=4000 + n + N + runs)
+    volt = synth.gauss_voltages(spec)
+    ref = oracle.fx(volt, N, K, T, F, 0)
+    monkeypatch.setenv("MWAX_X_EDGE", "1")
+    monkeypatch.setenv("MWAX_X_EDGE_RUNS", str(runs))
+    got = _run_fx(volt, n, N, K, T, F, 0)[0]
+    monkeypatch.setenv("MWAX_X_EDGE", "0")
+    plain = _run_fx(volt, n, N, K, T, F, 0)[0]
+    assert not np.isnan(got.view(np.float64)).any()
+    assert _norm_err(got, ref, n) <= TOL
+    assert _norm_err(plain, ref, n) <= TOL
+    assert _norm_err(got, plain, n) <= 1e-5        # same products, another summation order
+    ii = np.arange(n)
+    assert np.all(got[:, ii * (ii + 1) // 2 + ii].imag == 0.0)
+
+
+def test_shared_edge_schedule_with_streaming_accumulation(monkeypatch):
+    """MWAX_OPT_ACCUMULATE under the shared-edge schedule: two blocks added equal one integration."""
+    n, N, K, T, F = 16, 64, 64, 64, 2
+    spec = synth.GaussSpec(n, N * 2 * T, N, sigma=16.0, rho=0.2, tones=[], seed=4242)
+    volt = synth.gauss_voltages(spec)
+    ref = oracle.fx(volt, N, K, 2 * T, F, 0)
+    monkeypatch.setenv("MWAX_X_EDGE", "1")
+    monkeypatch.setenv("MWAX_X_EDGE_RUNS", "3")
+    h = corr.MwaxCorr(n, N, K, T, F)
+    v = torch.from_numpy(volt).cuda()
+    out = h.new_output()
+    out.fill_(float("nan"))
+    for b in range(2):
+        h.set_accumulate(b > 0)
+        h.process(v[:, b * T * N:(b + 1) * T * N].contiguous(), out[0, 0])
+    torch.cuda.synchronize()
+    got = _complex(out.cpu().numpy()[0, 0])
+    h.destroy()
+    assert _norm_err(got, ref, n) <= TOL
