@@ -30,13 +30,17 @@ UNIT = "coarse channels sustained in real time (whole job)"
 SAMPLE_RATE = 1.28e6
 
 
-def _executed_note(n: int, F: int) -> str:
+def _executed_note(n: int, F: int, C: int = 0, edge_runs: int = 0) -> str:
     """MMA work the X kernel issues per algorithmic flop: 256 x 256 pair tiles over the lower triangle of the 2n x 2n
-    real Gram matrix, times (F + 1) / F taps when F is even (shared edge channels)."""
+    real Gram matrix, times the fine channels contracted per output channel over F when F is even
+    (shared edge channels): (F + 1) / F in the plain schedule, (C F + runs) / (C F) in the shared-edge one."""
     m = (2 * n + 255) // 256
     tri = (m * (m + 1) // 2) * 65536 / (n * (2 * n + 1))
-    taps = (F + 1) / F if (F > 1 and F % 2 == 0) else 1.0
-    return (f"tiles cover {tri:.2f}x the lower triangle at n={n}" + (f", {taps:.2f}x taps at F={F}" if taps > 1 else "")
+    taps = 1.0
+    if F > 1 and F % 2 == 0:
+        taps = (C * F + edge_runs) / (C * F) if (edge_runs > 0 and C > 0) else (F + 1) / F
+    sched = f" (shared-edge schedule, {edge_runs} runs per tile)" if edge_runs > 0 else ""
+    return (f"tiles cover {tri:.2f}x the lower triangle at n={n}" + (f", {taps:.3f}x taps at F={F}{sched}" if taps > 1 else "")
             + " (DESIGN.md 5.2-5.3)")
 
 
@@ -231,6 +235,7 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e, do_next=True):
     torch.cuda.synchronize()
     data_seconds = data_seconds * NCO
     h = corr.MwaxCorr(n, N, K, T, F)
+    edge_runs = h.x_edge_runs()
     vis = h.new_output(n_dumps=D, n_coarse=NCO)
     stream = torch.cuda.current_stream()
     sp = int(stream.cuda_stream)
@@ -280,7 +285,7 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e, do_next=True):
     x_ms = [e[1].elapsed_time(e[2]) for s_ in evs for e in s_]
     f_avg_ms, x_avg_ms = sum(f_ms) / len(f_ms), sum(x_ms) / len(x_ms)
     res = {"cfg": cfg, "value": world * data_seconds / (ms_per_step * 1e-3), "ms_per_step": ms_per_step,
-           "total_ms": total_ms, "f_ms": f_avg_ms, "x_ms": x_avg_ms, "clocks": clocks,
+           "total_ms": total_ms, "f_ms": f_avg_ms, "x_ms": x_avg_ms, "clocks": clocks, "edge_runs": edge_runs,
            "launches": steps * D * NCO * h.launches_per_process(), "in_bytes": volt.numel(),
            "ws_bytes": h.workspace_bytes(), "e2e": None,
            "input_samples_per_s": world * n * row / (ms_per_step * 1e-3)}
@@ -393,7 +398,7 @@ def rooflines(res, peaks, traffic, wl):
               "unit": "TFLOP/s", "frac": x_ach / tensor_peak, "traffic": traffic.get((wl, "x")),
               "avg_launch_ms": res["x_ms"], "peak_source": f"{peaks['source']} bf16 {peak_kind} (MEASURED_PEAKS.json)",
               "frac_of_nominal_2250": x_ach / 2250.0,
-              "executed_over_algorithmic": _executed_note(n, cfg.f_avg)}
+              "executed_over_algorithmic": _executed_note(n, cfg.f_avg, K // cfg.f_avg, res.get("edge_runs", 0))}
     roof_f = {"kernel": f_name, "bound": "hbm", "achieved": f_ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
               "frac": f_ach / peaks["hbm_gbs"], "traffic": traffic.get((wl, "f")), "avg_launch_ms": res["f_ms"],
               "avg_launch_ms_with_delay_phase_correction": res.get("f_ms_delay"),

@@ -158,6 +158,11 @@ size_t mwax_corr_workspace_bytes(const mwax_corr_t *h);
  * least mwax_corr_workspace_bytes() bytes, 256-byte aligned; it is zeroed here, the library's own buffer is released,
  * and the memory must outlive the handle's last call.  Synchronises the device; not to be called with work in flight. */
 int mwax_corr_set_workspace(mwax_corr_t *h, void *d_ws, size_t bytes);
+/* X-stage schedule of this plan: with even f_avg and the centre-symmetric averaging of PAPER.md L290-298
+ * the outermost fine channel of an output channel is shared, at half weight, with its neighbour; when it pays, a CTA
+ * pair walks a run of adjacent output channels and contracts each shared channel once.  Returns the number of such runs
+ * per tile (> 0), 0 for the plain schedule (every output channel on its own), or a negative MWAX_ERR_* code. */
+int mwax_corr_x_edge_runs(mwax_corr_t *h);
 /* number of kernel launches one process() call enqueues */
 int mwax_corr_launches_per_process(const mwax_corr_t *h);
 int mwax_corr_last_cuda_error(const mwax_corr_t *h);

@@ -74,6 +74,7 @@ def lib() -> ctypes.CDLL:
         L.mwax_corr_f_stage.argtypes = [vp, vp, sz, vp]
         L.mwax_corr_set_delays.argtypes = [vp, vp, vp, sz, sz]
         L.mwax_corr_set_workspace.argtypes = [vp, vp, sz]
+        L.mwax_corr_x_edge_runs.argtypes = [vp]
         L.mwax_corr_set_channel_gains.argtypes = [vp, vp]
         L.mwax_corr_to_mwax_order.argtypes = [vp, vp, vp, vp, vp]
         L.mwax_corr_to_mwax_order_weighted.argtypes = [vp, vp, vp, i32, i32, vp, vp, vp]
@@ -134,6 +135,13 @@ class MwaxCorr:
         self._ws_ref = ws
         _check(lib().mwax_corr_set_workspace(self._h, ws.data_ptr(), ws.numel() * ws.element_size()), "mwax_corr_set_workspace",
                self._h)
+
+    def x_edge_runs(self) -> int:
+        """Runs per tile of the X stage's shared-edge schedule (even f_avg), 0 = plain schedule."""
+        r = lib().mwax_corr_x_edge_runs(self._h)
+        if r < 0:
+            _check(r, "mwax_corr_x_edge_runs", self._h)
+        return r
 
     def set_accumulate(self, on: bool):
         """Streaming integration: with True, process() adds into `vis` instead of overwriting it."""

@@ -611,6 +611,16 @@ int mwax_corr_set_delays(mwax_corr_t *h, const float *d_delay, const float *d_ph
     return MWAX_OK;
 }
 
+int mwax_corr_x_edge_runs(mwax_corr_t *h)
+{
+    if (!h) return MWAX_ERR_NULL;
+    if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
+    if (h->edge_runs < 0)
+        h->edge_runs = (h->x_pair && h->avg_mode == MWAX_AVG_CENTRE_SYMMETRIC && h->n_taps == h->F + 1)
+                           ? choose_edge_runs(h->C, h->F, h->T, h->n_ptiles, x_pair_capacity<false, true>(h->sm_count)) : 0;
+    return h->edge_runs;
+}
+
 int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
 {
     if (!h || !d_vis) return MWAX_ERR_NULL;
@@ -623,10 +633,7 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
     xp.edge_runs = 0;
     if (h->x_pair) {
         xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
-        if (h->edge_runs < 0)
-            h->edge_runs = (h->avg_mode == MWAX_AVG_CENTRE_SYMMETRIC && h->n_taps == h->F + 1)
-                               ? choose_edge_runs(h->C, h->F, h->T, h->n_ptiles, x_pair_capacity<false, true>(h->sm_count)) : 0;
-        xp.edge_runs = h->edge_runs;
+        xp.edge_runs = mwax_corr_x_edge_runs(h);
         int rcp = xp.edge_runs > 0 ? launch_x_pair<false, true>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream)
                                    : launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
         if (rcp != MWAX_OK) note_cuda(&h->last_cuda);
