@@ -10,6 +10,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <algorithm>
 #include <vector>
 
 #include "../../include/mwax_corr.h"
@@ -260,8 +261,12 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
 }
 
 // Shared-edge schedule (x_stage.cuh): how many runs of adjacent output channels per tile, or 0 when the
-// plain schedule is at least as good.  Cost model = waves of the persistent grid x taps of the longest unit: a run of L
-// channels contracts L F + 1 fine channels, the plain schedule F + 1 per channel.
+// plain schedule is at least as good.  Cost model = waves of the persistent grid x cost of the longest unit, in contraction
+// rows: an accumulator costs max(its rows, its epilogue), the epilogues measured on B200 as ~860 rows' worth of MMA time for
+// one that stores a 256 x 256 tile and ~770 for one that only updates the running sums (n = 512, F = 2, T = 64..512:
+// the plain schedule levels off at 0.09 ms below T = 256, the shared-edge one at 0.17 ms below T = 512).  A run of L channels
+// costs max(T, 770) + L max(F T, 860 + 770), the plain schedule max((F + 1) T, 860) per channel; the shared-edge kernel also
+// has 4 instead of 6 pipeline stages (F = 50: 3 % slower than the model says), hence the 4 % handicap and the 8 % margin.
 // MWAX_X_EDGE=0 never, =1 whenever the geometry allows it (tests); MWAX_X_EDGE_RUNS forces the run count.
 int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs)
 {
@@ -269,16 +274,20 @@ int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs)
     if (const char *e = getenv("MWAX_X_EDGE")) force = atoi(e);
     if (force == 0 || F < 2 || (F & 1) || T < 64 || pairs < 1) return 0;
     if (const char *e = getenv("MWAX_X_EDGE_RUNS")) { const int v = atoi(e); if (v >= 1 && v <= C) return v; }
-    const long long plain = (((long long)C * n_tiles + pairs - 1) / pairs) * (F + 1);
+    const long long e_out = 860, e_add = 770;
+    const long long per_chan_plain = std::max<long long>((long long)(F + 1) * T, e_out);
+    const long long per_chan_edge = std::max<long long>((long long)F * T, e_out + e_add);
+    const long long init = std::max<long long>(T, e_add);
+    const long long plain = (((long long)C * n_tiles + pairs - 1) / pairs) * per_chan_plain;
     long long best = -1;
     int best_r = 0;
     for (int r = 1; r <= C; ++r) {
         const long long waves = ((long long)r * n_tiles + pairs - 1) / pairs;
-        const long long cost = waves * ((long long)((C + r - 1) / r) * F + 1);
+        const long long cost = waves * (init + (long long)((C + r - 1) / r) * per_chan_edge);
         if (best < 0 || cost < best) { best = cost; best_r = r; }
     }
     if (force == 1) return best_r;
-    return (best * 100 <= plain * 92) ? best_r : 0;
+    return (best * 104 <= plain * 92) ? best_r : 0;
 }
 
 }  // namespace
