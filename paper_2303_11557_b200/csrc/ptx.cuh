@@ -131,6 +131,14 @@ __device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar)
 {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
 }
+// The same without release semantics.  `.release.cluster` compiles to MEMBAR.ALL.GPU + ERRBAR in front of the arrive, i.e. it
+// waits until every global store the thread has issued is acknowledged: for an epilogue warp handing its TMEM accumulator
+// back that is its whole output tile (ncu, short integrations: 19 % of the epilogue's stall samples on that ERRBAR).  What
+// the hand-over must order is the TMEM reads, and those are complete once tcgen05.wait::ld has returned.
+__device__ __forceinline__ void mbar_arrive_cluster_relaxed(uint32_t cluster_bar)
+{
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
 // TMA load issued by either CTA of a pair: data lands in THIS CTA's shared memory, the transaction bytes are
 // counted on `cluster_bar`, which may live in the other CTA of the pair (the leader's full barrier)
 __device__ __forceinline__ void tma_load_3d_pair(uint32_t dst, const CUtensorMap *m, int c0, int c1, int c2, uint32_t cluster_bar)

@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
                 x_epilogue_tile<kInt8, kEdge>(P, stg, t_row, c, i_base, nj * 128, C::BN / 32, sc, lane, mode, S);
                 ptx::tc_fence_before();
                 __syncwarp();
-                if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(as), 0));
+                if (lane == 0) ptx::mbar_arrive_cluster_relaxed(ptx::mapa(tempty_bar(as), 0));
                 if (++as == C::ACC_STAGES) { as = 0; aph ^= 1u; }
             });
         } else
@@ -281,7 +281,7 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
             x_epilogue_tile<kInt8>(P, stg, t_row, c, i_base, nj * 128, C::BN / 32, sc, lane);
             ptx::tc_fence_before();
             __syncwarp();
-            if (lane == 0) ptx::mbar_arrive_cluster(ptx::mapa(tempty_bar(as), 0));
+            if (lane == 0) ptx::mbar_arrive_cluster_relaxed(ptx::mapa(tempty_bar(as), 0));
             if (++as == C::ACC_STAGES) { as = 0; aph ^= 1u; }
         }
     }
