@@ -294,7 +294,16 @@ __global__ void __launch_bounds__(F6400P3::THREADS, 1) f_stage_6400p3_kernel(con
             ptx::fence_proxy_async();                                // the staged rows will be read by bulk copies
             if (threadIdx.x == 0) ptx::mbar_arrive_expect_tx(rx_bar_a, 400u * 128u);   // this item's incoming rows
         }
-        cluster_arrive();
+        // PUSH: the staged rows are read by THIS CTA's own bulk copies, so CTA-level ordering (bar.sync) is enough, and the
+        // cluster barrier only has to say "my pass 3 no longer reads the slots you are about to overwrite": a relaxed
+        // arrive.  The release form compiles to MEMBAR.ALL.GPU + ERRBAR, which also waits for the 20 voltage loads of the
+        // next item that were issued when pass 3 started - it turned the one-item-ahead prefetch into a blocking load.
+        if (PUSH) {
+            __syncthreads();
+            cluster_arrive_relaxed();
+        } else {
+            cluster_arrive();
+        }
         cluster_wait();                                              // every CTA of the cluster has staged its rows
         if (PUSH) {
             // rows of the OTHER CTA's k3 half: rank 0 sends its k3 >= 8 rows (input 3's slots), rank 1 its k3 < 8 rows
