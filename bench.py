@@ -201,7 +201,10 @@ def load_traffic():
             for ln in f:
                 if ln.startswith("#") or not ln.strip():
                     continue
-                w, stage, _k, b = [x.strip() for x in ln.split(",")][:4]
+                parts = [x.strip() for x in ln.split(",")]      # a kernel name may hold commas: bytes = last field
+                if len(parts) < 4:
+                    continue
+                w, stage, b = parts[0], parts[1], parts[-1]
                 try:
                     out[(w, stage)] = float(b)
                 except ValueError:
