@@ -336,6 +336,8 @@ struct mwax_corr {
     size_t d_row_stride, d_coarse_stride;
     cudaStream_t s_in, s_out;              // copy streams of process_host
     cudaEvent_t ev_start, ev_copied;
+    cudaEvent_t ev_part[8];                // channel ranges of the last dump of process_host
+    int host_tail_parts;
     std::vector<cudaEvent_t> ev_in, ev_done;
 };
 
@@ -630,19 +632,24 @@ int mwax_corr_x_edge_runs(mwax_corr_t *h)
     return h->edge_runs;
 }
 
-int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
+// X stage over the output channels [c0, c0 + cnt) of one dump (d_vis = the dump's base).  The kernels index their
+// per-channel tables and the output by channel number, so a sub-range is the same launch on offset pointers; the
+// shared-edge schedule walks runs of the whole channel axis and is used for the full range only.
+static int x_stage_range(mwax_corr_t *h, float *d_vis, int c0, int cnt, void *stream)
 {
     if (!h || !d_vis) return MWAX_ERR_NULL;
-    if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
+    if (!h->tables_ready || c0 < 0 || cnt < 1 || c0 + cnt > h->C) return MWAX_ERR_INVALID_ARG;
+    const bool whole = (c0 == 0 && cnt == h->C);
     mwax::XParams xp;
-    xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = h->C; xp.n_tiles = h->n_tiles;
-    xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = h->n_taps; xp.scale = h->d_scale;
-    xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = cnt; xp.n_tiles = h->n_tiles;
+    xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start + c0; xp.n_taps = h->n_taps; xp.scale = h->d_scale + c0;
+    xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    xp.out = d_vis + (size_t)c0 * (size_t)xp.out_chan_stride * 2;
     xp.accumulate = h->accumulate;
     xp.edge_runs = 0;
     if (h->x_pair) {
         xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
-        xp.edge_runs = mwax_corr_x_edge_runs(h);
+        xp.edge_runs = whole ? mwax_corr_x_edge_runs(h) : 0;
         int rcp = xp.edge_runs > 0 ? launch_x_pair<false, true>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream)
                                    : launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
         if (rcp != MWAX_OK) note_cuda(&h->last_cuda);
@@ -652,6 +659,12 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
                               : launch_x<false, 256>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
     if (rc != MWAX_OK) note_cuda(&h->last_cuda);
     return rc;
+}
+
+int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream)
+{
+    if (!h) return MWAX_ERR_NULL;
+    return x_stage_range(h, d_vis, 0, h->C, stream);
 }
 
 int mwax_corr_process_batch(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, size_t coarse_pitch, int n_dumps,
@@ -716,6 +729,10 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
         if (cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&h->ev_copied, cudaEventDisableTiming) != cudaSuccess)
             return note_cuda(&h->last_cuda);
+        for (int q = 0; q < 8; ++q)
+            if (cudaEventCreateWithFlags(&h->ev_part[q], cudaEventDisableTiming) != cudaSuccess) return note_cuda(&h->last_cuda);
+        h->host_tail_parts = 4;
+        if (const char *pe = getenv("MWAX_HOST_TAIL_PARTS")) { const int v = atoi(pe); if (v >= 1 && v <= 8) h->host_tail_parts = v; }
     }
     // the copy streams start after whatever the caller has already queued on `stream`
     cudaEventRecord(h->ev_start, st);
@@ -737,13 +754,22 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
             if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)(d + 1) * h->T) return MWAX_ERR_INVALID_ARG;
             int rc = f_stage_impl(h, h->d_in + 2 * d * dump_samples, row_samples, d * h->T, c, st);
             if (rc != MWAX_OK) return rc;
-            rc = mwax_corr_x_stage(h, h->d_out + (size_t)d * vis_floats, st);
-            if (rc != MWAX_OK) return rc;
-            cudaEventRecord(h->ev_done[e], st);
-            cudaStreamWaitEvent(h->s_out, h->ev_done[e], 0);
-            if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c * out_bytes + (size_t)d * dump_out,
-                                h->d_out + (size_t)d * vis_floats, dump_out, cudaMemcpyDeviceToHost, h->s_out) != cudaSuccess)
-                return note_cuda(&h->last_cuda);
+            // Nothing hides the device -> host copy of the LAST dump: it is correlated in `parts` channel ranges and each
+            // range leaves while the next is computed (plain schedule only; earlier dumps travel under the next dump's work).
+            int parts = 1;
+            if (e == n_ev - 1 && !h->accumulate && h->C >= 8 && !(h->x_pair && mwax_corr_x_edge_runs(h) > 0)) parts = h->host_tail_parts;
+            for (int q = 0; q < parts; ++q) {
+                const int c0 = (int)(((long long)q * h->C) / parts), c1 = (int)(((long long)(q + 1) * h->C) / parts);
+                rc = x_stage_range(h, h->d_out + (size_t)d * vis_floats, c0, c1 - c0, st);
+                if (rc != MWAX_OK) return rc;
+                cudaEventRecord(q == parts - 1 ? h->ev_done[e] : h->ev_part[q], st);
+                cudaStreamWaitEvent(h->s_out, q == parts - 1 ? h->ev_done[e] : h->ev_part[q], 0);
+                const size_t off = (size_t)c0 * (dump_out / h->C), len = (size_t)(c1 - c0) * (dump_out / h->C);
+                if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c * out_bytes + (size_t)d * dump_out + off,
+                                    reinterpret_cast<char *>(h->d_out + (size_t)d * vis_floats) + off, len, cudaMemcpyDeviceToHost,
+                                    h->s_out) != cudaSuccess)
+                    return note_cuda(&h->last_cuda);
+            }
             if (d == n_dumps - 1) cudaEventRecord(h->ev_copied, h->s_out);
         }
     // join: the caller's stream continues after the last copy; the call itself returns when everything has landed
@@ -818,6 +844,7 @@ int mwax_corr_destroy(mwax_corr_t *h)
     for (cudaEvent_t e : h->ev_done) cudaEventDestroy(e);
     if (h->ev_start) cudaEventDestroy(h->ev_start);
     if (h->ev_copied) cudaEventDestroy(h->ev_copied);
+    for (cudaEvent_t e : h->ev_part) if (e) cudaEventDestroy(e);
     if (h->s_in) cudaStreamDestroy(h->s_in);
     if (h->s_out) cudaStreamDestroy(h->s_out);
     delete h;

@@ -255,16 +255,21 @@ def test_fx_config5_shape_two_coarse_channels_sampled():
             assert _norm_err(_gather_sel(got[c, d], sel), ref, len(sel)) <= TOL
 
 
-def test_host_buffer_entry_matches_device_entry():
-    n, N, T, D = 32, 128, 20, 2
-    spec = synth.GaussSpec(n, N * T * D, N, sigma=16.0, rho=0.1, seed=9)
-    volt = synth.gauss_voltages(spec)
-    h = corr.MwaxCorr(n, N, N, T, 2)
-    dev = h.new_output(n_dumps=D)
-    h.process_batch(torch.from_numpy(volt)[None].cuda(), dev, D)
-    hv = torch.from_numpy(volt)[None].contiguous().pin_memory()
-    hout = torch.empty(dev.shape, dtype=torch.float32).pin_memory()
-    h.process_host(hv, hout, D)
+@pytest.mark.parametrize("n,N,K,T,F,D,NCO", [
+    (32, 128, 128, 20, 2, 2, 1),
+    (70, 320, 300, 6, 3, 1, 2),      # two coarse channels through the reused staging; 100 output channels in 4 uneven ranges
+    (300, 64, 64, 40, 1, 3, 1),      # pair tiles; the last dump leaves in channel ranges (mwax_api.cu: process_host)
+    (20, 64, 6, 12, 1, 2, 1),        # fewer than 8 output channels: no ranges
+])
+def test_host_buffer_entry_matches_device_entry(n, N, K, T, F, D, NCO):
+    volt = np.stack([synth.gauss_voltages(synth.GaussSpec(n, N * T * D, N, sigma=16.0, rho=0.1, seed=9 + c))
+                     for c in range(NCO)])
+    h = corr.MwaxCorr(n, N, K, T, F)
+    dev = h.new_output(n_dumps=D, n_coarse=NCO)
+    h.process_batch(torch.from_numpy(volt).cuda(), dev, D, NCO)
+    hv = torch.from_numpy(volt).contiguous().pin_memory()
+    hout = torch.full(dev.shape, float("nan"), dtype=torch.float32).pin_memory()
+    h.process_host(hv, hout, D, NCO)
     torch.cuda.synchronize()
     assert torch.equal(hout, dev.cpu())
     h.destroy()
