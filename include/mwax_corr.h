@@ -121,8 +121,12 @@ int mwax_corr_process_batch(mwax_corr_t *h, const int8_t *d_volt, size_t row_pit
                             int n_dumps, int n_coarse, float *d_vis, void *stream);
 
 /* Same as process_batch but with HOST buffers (pinned memory recommended): the call copies the voltages
- * host->device, runs the path, copies the visibilities device->host, all on `stream`, and synchronises
- * the stream before returning.  Staging buffers are owned by the handle (allocated on first use). */
+ * host->device, runs the path, copies the visibilities device->host and synchronises `stream` before
+ * returning.  The kernels run on `stream`, after whatever the caller has queued there; the copies run on two
+ * streams of the handle so that dump d + 1 arrives and dump d - 1 leaves while dump d is correlated (the last
+ * dump leaves in channel ranges).  Staging buffers are owned by the handle (allocated on first use).
+ * Errors: MWAX_ERR_NULL, MWAX_ERR_INVALID_ARG (pitch shorter than n_dumps integrations), MWAX_ERR_NOMEM
+ * (staging), MWAX_ERR_CUDA. */
 int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitch, size_t coarse_pitch,
                            int n_dumps, int n_coarse, float *h_vis, void *stream);
 
