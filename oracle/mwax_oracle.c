@@ -33,6 +33,7 @@ typedef double complex cplx;
 
 #define AVG_CENTRE_SYMMETRIC 0
 #define AVG_BLOCK 1
+#define AVG_KEEP_DC 2 /* flag, OR-ed into the centre-symmetric mode: do NOT exclude the DC ultra-fine channel */
 
 static const double TWO_PI = 6.283185307179586476925286766559;
 
@@ -125,6 +126,10 @@ int mwax_oracle_fft(int N, const double *in_ri, double *out_ri)
  *    F/(F-1) (L290-294; Q6, Q7);
  *  - finally a mean: all weights divided by F (Q5).
  *  BLOCK mode (legacy adjacent grouping, Fig 6a): W[c][p] = 1/F for p in [cF,(c+1)F).
+ *  AVG_KEEP_DC (flag on the centre-symmetric mode; SURVEY.md 8(b) MWAX_OPT_DC_EXCLUDE = 0): L290-294 describe the
+ *  exclusion as something the averaging step DOES ("That centre ultra-fine channel is excluded ... and the output
+ *  re-scaled accordingly"); with the flag the step is left out: the DC tap keeps weight 1 and the centre channel is a
+ *  plain mean like every other channel (no F/(F-1)).
  *  Position p <-> signed bin u = p - floor(K/2) (step 3). */
 int mwax_oracle_weights(int K, int F, int mode, double *W)
 {
@@ -136,7 +141,8 @@ int mwax_oracle_weights(int K, int F, int mode, double *W)
             for (int p = c * F; p < (c + 1) * F; ++p) W[(size_t)c * K + p] = 1.0 / F;
         return ORACLE_OK;
     }
-    if (mode != AVG_CENTRE_SYMMETRIC) return ORACLE_ERR_ARG;
+    if (mode != AVG_CENTRE_SYMMETRIC && mode != (AVG_CENTRE_SYMMETRIC | AVG_KEEP_DC)) return ORACLE_ERR_ARG;
+    const int dc_exclude = !(mode & AVG_KEEP_DC);
     const int c0 = C / 2, half = K / 2;
     for (int c = 0; c < C; ++c) {
         const int uc = (c - c0) * F;
@@ -146,10 +152,10 @@ int mwax_oracle_weights(int K, int F, int mode, double *W)
             if (F % 2 == 0 && (delta == -dmax || delta == dmax)) wt = 0.5;
             int u = uc + delta;
             int p = ((u + half) % K + K) % K;
-            if (F > 1 && c == c0 && delta == 0) wt = 0.0; /* DC excluded */
+            if (dc_exclude && F > 1 && c == c0 && delta == 0) wt = 0.0; /* DC excluded */
             W[(size_t)c * K + p] += wt;
         }
-        if (F > 1 && c == c0)
+        if (dc_exclude && F > 1 && c == c0)
             for (int p = 0; p < K; ++p) W[(size_t)c * K + p] *= (double)F / (double)(F - 1);
         for (int p = 0; p < K; ++p) W[(size_t)c * K + p] /= (double)F;
     }

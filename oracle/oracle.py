@@ -19,6 +19,7 @@ _lib = None
 
 AVG_CENTRE_SYMMETRIC = 0
 AVG_BLOCK = 1
+AVG_KEEP_DC = 2   # flag on the centre-symmetric mode: the DC ultra-fine channel is NOT excluded (PAPER.md L290-294 left out)
 
 
 def build(force: bool = False) -> str:

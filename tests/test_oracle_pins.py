@@ -260,6 +260,39 @@ def test_p8_dc_tone_vanishes_and_white_noise_is_flat():
     assert abs(V[c0] / np.delete(V, c0).mean() - 1.0) < 0.05
 
 
+@pytest.mark.parametrize("K,F", [(8, 2), (64, 4), (75, 3), (6400, 50)])
+def test_keep_dc_mode_weights(K, F):
+    """MWAX_OPT_DC_EXCLUDE = 0: the exclusion of PAPER.md L290-294 left out.  Every fine channel then
+    has total weight exactly 1 across the outputs (partition of unity with NO exception), every row is a mean, the
+    centre row is the mirror-symmetric F (odd) / F + 1 (even, half-weight ends) tap window around DC written out here,
+    and all other rows equal those of the default mode."""
+    W = oracle.weights(K, F, oracle.AVG_KEEP_DC)
+    Wd = oracle.weights(K, F)
+    C, dc = K // F, K // 2
+    c0 = C // 2
+    assert np.allclose(W.sum(axis=1), 1.0) and np.allclose(W.sum(axis=0) * F, 1.0)
+    expect = np.zeros(K)
+    dmax = (F - 1) // 2 if F % 2 else F // 2
+    for d in range(-dmax, dmax + 1):
+        expect[(dc + d) % K] += (0.5 if (F % 2 == 0 and abs(d) == dmax) else 1.0) / F
+    assert np.allclose(W[c0], expect)
+    assert np.array_equal(np.delete(W, c0, axis=0), np.delete(Wd, c0, axis=0))
+
+
+def test_keep_dc_mode_dc_tone_survives():
+    """The pair to test_p8: with the exclusion off a DC offset of amplitude A appears in the centre channel only, at
+    its closed-form power T (A N)^2 / F (one of the F taps of the mean holds it); with it on (default) it vanishes."""
+    N = K = 64
+    F, T, A = 4, 4, 50.0
+    x = np.full(N * T, A + 0j)
+    volt = _volt_from_complex(x[None, :])
+    V = oracle.fx(volt, N, K, T, F, oracle.AVG_KEEP_DC)[:, 0].real
+    c0 = (K // F) // 2
+    assert abs(V[c0] / (T * (A * N) ** 2 / F) - 1.0) < 1e-12
+    assert np.abs(np.delete(V, c0)).max() < 1e-6
+    assert np.abs(oracle.fx(volt, N, K, T, F)[:, 0]).max() < 1e-6
+
+
 def test_block_mode_weights():
     W = oracle.weights(12, 3, oracle.AVG_BLOCK)
     for c in range(4):
