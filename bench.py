@@ -273,10 +273,12 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e, do_next=True):
     sampler.start()
     t_start = torch.cuda.Event(enable_timing=True)
     t_end = torch.cuda.Event(enable_timing=True)
+    launches0 = h.launch_count()
     t_start.record(stream)
     for k in range(steps):
         step(evs[k])
     t_end.record(stream)
+    launches = h.launch_count() - launches0          # counted by the library: every kernel it enqueued in the timed region
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
@@ -289,7 +291,7 @@ def measure(wl, steps, warmup, world, rank, local_rank, do_e2e, do_next=True):
     f_avg_ms, x_avg_ms = sum(f_ms) / len(f_ms), sum(x_ms) / len(x_ms)
     res = {"cfg": cfg, "value": world * data_seconds / (ms_per_step * 1e-3), "ms_per_step": ms_per_step,
            "total_ms": total_ms, "f_ms": f_avg_ms, "x_ms": x_avg_ms, "clocks": clocks, "edge_runs": edge_runs,
-           "launches": steps * D * NCO * h.launches_per_process(), "in_bytes": volt.numel(),
+           "launches": launches, "in_bytes": volt.numel(),
            "ws_bytes": h.workspace_bytes(), "e2e": None,
            "input_samples_per_s": world * n * row / (ms_per_step * 1e-3)}
 
@@ -396,7 +398,7 @@ def rooflines(res, peaks, traffic, wl):
     tensor_peak = peaks["tensor_sustained"] if peak_kind == "sustained" else peaks["tensor_burst"]
     x_ach = 8.0 * B * K * T / (res["x_ms"] * 1e-3) / 1e12
     f_ach = (n * T * N * 2.0 + n * T * K * 4.0) / (res["f_ms"] * 1e-3) / 1e9
-    f_name = {6400: "f_stage_6400p3_kernel"}.get(N, "f_stage_pow2_kernel" if N in (64, 128, 256, 512) else "f_stage_generic_kernel")
+    f_name = {6400: "f_stage_6400_kernel"}.get(N, "f_stage_pow2_kernel" if N in (64, 128, 256, 512) else "f_stage_generic_kernel")
     roof_x = {"kernel": "x_stage_pair_kernel<fp16> (cta_group::2, 256x256 tiles)", "bound": "tensor", "achieved": x_ach, "peak": tensor_peak,
               "unit": "TFLOP/s", "frac": x_ach / tensor_peak, "traffic": traffic.get((wl, "x")),
               "avg_launch_ms": res["x_ms"], "peak_source": f"{peaks['source']} bf16 {peak_kind} (MEASURED_PEAKS.json)",

@@ -22,7 +22,11 @@
  *
  * Threading/streams: all device work of a call is enqueued on `stream` (a cudaStream_t passed as void*;
  * NULL = the legacy default stream) and the call returns after enqueueing.  One call in flight per handle
- * (the handle owns a workspace); different handles may run on different streams.
+ * (the handle owns a workspace); different handles may run on different streams and threads.
+ * Devices: a handle belongs to the CUDA device that was current when it was created (any sm_100 device of the
+ * process; the library is built for sm_100a only, other architectures get MWAX_ERR_ARCH).  Every call must be made
+ * with that device current, otherwise it returns MWAX_ERR_INVALID_ARG without enqueueing anything.
+ * The library reads no environment variables: every knob is an argument or a mwax_corr_set_option key below.
  */
 #ifndef MWAX_CORR_H
 #define MWAX_CORR_H
@@ -48,7 +52,7 @@ enum {
 };
 
 /* options for mwax_corr_set_option */
-enum { MWAX_OPT_AVG_MODE = 1, MWAX_OPT_ACCUMULATE = 2 };
+enum { MWAX_OPT_AVG_MODE = 1, MWAX_OPT_ACCUMULATE = 2, MWAX_OPT_DC_EXCLUDE = 3, MWAX_OPT_X_EDGE_RUNS = 4 };
 enum { MWAX_AVG_CENTRE_SYMMETRIC = 0, MWAX_AVG_BLOCK = 1 };
 
 /* ------------------------------------------------------------------------------------------------------
@@ -68,6 +72,14 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
 int mwax_corr_last_error(void);
 
 /* MWAX_OPT_AVG_MODE: averaging geometry; call before the first process().  Default MWAX_AVG_CENTRE_SYMMETRIC (L290).
+ * MWAX_OPT_DC_EXCLUDE (1/0, default 1; centre-symmetric mode, f_avg > 1): "That centre ultra-fine channel
+ *   is excluded ... and the output re-scaled accordingly".  With 1 the DC fine channel gets weight 0 in the centre output
+ *   channel, which is multiplied by F/(F-1); with 0 the step is left out: the DC fine channel is averaged in like any
+ *   other and the centre channel is a plain mean.  Rebuilds the small device tables (synchronous).
+ * MWAX_OPT_X_EDGE_RUNS (default -1): schedule of the X stage when f_avg is even (see mwax_corr_x_edge_runs): -1 = the
+ *   library decides from its cost model, 0 = never use the shared-edge schedule, r >= 1 = use it with r runs of adjacent
+ *   output channels per tile (clamped to C) whenever the geometry allows it (even f_avg, centre-symmetric, t_int >= 64).
+ *   A scheduling knob only: every setting computes the same sums (in a different fp32 order).
  * MWAX_OPT_ACCUMULATE (0/1, default 0): streaming integration (§2.5, §2.5.2:
  *   50 ms blocks aggregated into the integration).  With 1, process()/process_batch()/x_stage() ADD their result to
  *   what d_vis already holds, so an integration of any length is the sum of calls over its pieces (t_int = spectra per
@@ -143,7 +155,10 @@ int mwax_corr_x_stage(mwax_corr_t *h, float *d_vis, void *stream);
  *                   (0-0, 0-1, ..., 0-(nt-1), 1-1, ...); element (antA, antB, ch, pq) = sum X_{antA,p} conj(X_{antB,q})
  *                   (reading Q21).  mwax_corr_mwax_order_bytes() bytes.
  *   d_weights  out: float [n_tiles(n_tiles+1)/2][4] visibility weights, all 1.0 (L328), or NULL
- * Pure data movement: the values are bit copies (sign of Im flipped where the conjugate is taken). */
+ * Pure data movement: the values are bit copies (sign of Im flipped where the conjugate is taken).
+ * CAVEAT (readings Q2, Q21, both "parity unpinned"): PAPER.md does not say which antenna of a baseline is
+ * conjugated nor how Fig. 8's xx, xy, yx, yy map onto (antA, antB); nothing in the container pins it.  The output may
+ * therefore be the complex conjugate (and xy/yx swapped) of what the real instrument writes. */
 int mwax_corr_to_mwax_order(mwax_corr_t *h, const float *d_vis, float *d_out, float *d_weights, void *stream);
 size_t mwax_corr_mwax_order_bytes(const mwax_corr_t *h);
 
@@ -167,18 +182,23 @@ int mwax_corr_set_workspace(mwax_corr_t *h, void *d_ws, size_t bytes);
  * pair walks a run of adjacent output channels and contracts each shared channel once.  Returns the number of such runs
  * per tile (> 0), 0 for the plain schedule (every output channel on its own), or a negative MWAX_ERR_* code. */
 int mwax_corr_x_edge_runs(mwax_corr_t *h);
-/* number of kernel launches one process() call enqueues */
-int mwax_corr_launches_per_process(const mwax_corr_t *h);
+/* total number of kernels this handle has enqueued since create() (F, X and MWAX_ORDER kernels of every entry point) */
+long long mwax_corr_launch_count(const mwax_corr_t *h);
 int mwax_corr_last_cuda_error(const mwax_corr_t *h);
 int mwax_corr_destroy(mwax_corr_t *h); /* NULL is a no-op returning MWAX_OK */
 
 /* ------------------------------------------------------------------------------------------------------
  * X-only integer path (BASELINE.json configs[1]): the X-stage contraction on pre-channelised int8
  * samples, exact int32 accumulation, no FFT, no averaging.
- *   d_z   in : int8 [n_chan][n_time][n_inputs][re,im]; n_inputs must be a multiple of 8 (TMA needs a
- *              16-byte row pitch) and d_z 16-byte aligned
+ *   d_z   in : int8 [n_chan][n_time][n_inputs][re,im], any n_inputs >= 1.  The kernel reads the buffer in place through a
+ *              TMA tensor map when rows are 16-byte multiples (n_inputs % 8 == 0) and d_z is 16-byte aligned; otherwise
+ *              the call first copies it, on the device, into an internal buffer with rows padded to 16 bytes (one extra
+ *              pass over the input; allocated on first use, MWAX_ERR_NOMEM if that fails).  Partial tiles are padded by
+ *              the tensor map's out-of-bounds zero fill.
  *   d_vis out: int32 [n_chan][n(n+1)/2][re,im],  Re = sum(a_i a_j + b_i b_j), Im = sum(b_i a_j - a_i b_j)
- * The caller guarantees 2*128*128*n_time < 2^31 (n_time <= 65535) so int32 cannot overflow.
+ * The caller guarantees 2*128*128*n_time < 2^31 (n_time <= 65535, else MWAX_ERR_UNSUPPORTED) so int32 cannot overflow.
+ * process_host: the same with HOST buffers (pinned recommended); channels travel in 4 ranges so that range q + 1 goes
+ * host->device and range q - 1 device->host while range q is correlated; synchronises `stream` before returning.
  * ---------------------------------------------------------------------------------------------------- */
 mwax_xcorr_t *mwax_xcorr_i8_create(int n_inputs, int n_chan, int n_time);
 int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, void *stream);

@@ -15,13 +15,15 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 _LIB = os.path.join(_HERE, "libmwax_corr.so")
-_SOURCES = ["mwax_api.cu", "mwax_order.cuh", "f_stage.cuh", "f_stage_pow2.cuh", "f_stage_6400p3.cuh", "x_stage.cuh", "x_stage2.cuh", "ptx.cuh"]
+_SOURCES = ["mwax_api.cu", "mwax_order.cuh", "f_stage.cuh", "f_stage_pow2.cuh", "f_stage_6400.cuh", "x_stage.cuh", "x_stage2.cuh", "ptx.cuh"]
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "mwax_corr.h")
 _lib = None
 
 MWAX_OK = 0
 MWAX_OPT_AVG_MODE = 1
 MWAX_OPT_ACCUMULATE = 2
+MWAX_OPT_DC_EXCLUDE = 3
+MWAX_OPT_X_EDGE_RUNS = 4
 MWAX_AVG_CENTRE_SYMMETRIC = 0
 MWAX_AVG_BLOCK = 1
 
@@ -84,7 +86,8 @@ def lib() -> ctypes.CDLL:
         for f in ("input_bytes", "output_bytes", "workspace_bytes"):
             getattr(L, "mwax_corr_" + f).restype = sz
             getattr(L, "mwax_corr_" + f).argtypes = [vp]
-        L.mwax_corr_launches_per_process.argtypes = [vp]
+        L.mwax_corr_launch_count.restype = ctypes.c_longlong
+        L.mwax_corr_launch_count.argtypes = [vp]
         L.mwax_corr_last_cuda_error.argtypes = [vp]
         L.mwax_corr_destroy.argtypes = [vp]
         L.mwax_xcorr_i8_create.restype = vp
@@ -157,8 +160,13 @@ class MwaxCorr:
     def workspace_bytes(self) -> int:
         return lib().mwax_corr_workspace_bytes(self._h)
 
-    def launches_per_process(self) -> int:
-        return lib().mwax_corr_launches_per_process(self._h)
+    def launch_count(self) -> int:
+        """Kernels this handle has enqueued since it was created."""
+        return int(lib().mwax_corr_launch_count(self._h))
+
+    def set_option(self, key: int, value: int):
+        """mwax_corr_set_option: MWAX_OPT_AVG_MODE, MWAX_OPT_ACCUMULATE, MWAX_OPT_DC_EXCLUDE, MWAX_OPT_X_EDGE_RUNS."""
+        _check(lib().mwax_corr_set_option(self._h, key, value), "mwax_corr_set_option", self._h)
 
     def new_output(self, n_dumps: int = 1, n_coarse: int = 1, device="cuda") -> torch.Tensor:
         return torch.empty((n_coarse, n_dumps, self.n_out, self.n_baselines, 2), dtype=torch.float32, device=device)

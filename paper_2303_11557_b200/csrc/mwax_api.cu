@@ -11,12 +11,14 @@
 #include <cstring>
 #include <new>
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <vector>
 
 #include "../../include/mwax_corr.h"
 #include "f_stage.cuh"
 #include "f_stage_pow2.cuh"
-#include "f_stage_6400p3.cuh"
+#include "f_stage_6400.cuh"
 #include "x_stage.cuh"
 #include "x_stage2.cuh"
 #include "mwax_order.cuh"
@@ -69,35 +71,28 @@ bool factor_2_5(int N, std::vector<int> &radix)
     return N == 1;
 }
 
-int check_device(int *sm_count)
+// The library is built for sm_100a only (arch-specific code, not forward compatible): any other device, sm_103 included,
+// is refused here instead of failing at the first launch with "no kernel image".
+int check_device(int *sm_count, int *device)
 {
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return MWAX_ERR_ARCH;
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return MWAX_ERR_ARCH;
-    if (prop.major != 10) return MWAX_ERR_ARCH;
-    *sm_count = prop.multiProcessorCount;
+    int major = 0, minor = 0, sms = 0;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return MWAX_ERR_ARCH;
+    if (major != 10 || minor != 0) return MWAX_ERR_ARCH;
+    *sm_count = sms;
+    *device = dev;
     return MWAX_OK;
 }
 
-// lower-triangle tile list, 4 bytes per tile (mi, nj, w, 0): G rows of inputs [64 mi, 64 mi + 64), G columns of inputs
-// [64 nj, 64 nj + 64 w).  Row block mi needs the columns of inputs [0, 64 (mi + 1)): pairs of 64-input units become
-// 256-wide tiles (w = 2), an odd unit left over on the diagonal a 128-wide one (w = 1), so at n = 512 the tiles cover
-// 1.12x the lower triangle (16 wide + 4 narrow) instead of 1.25x (20 wide).
-void build_tiles(int n, int bn, std::vector<uint8_t> &tiles)
+// every entry point that launches work checks that the caller is on the device the handle was created on
+bool on_device(int device)
 {
-    tiles.clear();
-    for (int mi = 0; mi * 64 < n; ++mi) {
-        const int units = mi + 1;
-        for (int u = 0; u < units;) {
-            const int w = (bn == 256 && u + 2 <= units) ? 2 : 1;
-            tiles.push_back((uint8_t)mi);
-            tiles.push_back((uint8_t)u);
-            tiles.push_back((uint8_t)w);
-            tiles.push_back(0);
-            u += w;
-        }
-    }
+    int dev = -1;
+    return cudaGetDevice(&dev) == cudaSuccess && dev == device;
 }
 
 // tile list of the CTA-pair kernel: (mi, nj, 0, 0) in units of 128 inputs, nj <= mi
@@ -113,13 +108,6 @@ void build_pair_tiles(int n, std::vector<uint8_t> &tiles)
         }
 }
 
-int want_pair_kernel()
-{
-    // debugging aid: MWAX_X_PAIR=0 selects the single-CTA kernel instead of the cta_group::2 pair kernel
-    const char *e = getenv("MWAX_X_PAIR");
-    return (e && atoi(e) == 0) ? 0 : 1;
-}
-
 template <typename T>
 int upload(T **dptr, const std::vector<T> &h)
 {
@@ -129,23 +117,83 @@ int upload(T **dptr, const std::vector<T> &h)
     return MWAX_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ per-device setup
+// cudaFuncSetAttribute and the occupancy queries are per DEVICE, a handle may be created on any sm_100 device of the
+// process and handles may be used from different threads: the attributes of every kernel are set once per device, under
+// a mutex, before create() returns; the launch paths only read what the handle copied from here.
+constexpr int HOST_PARTS = 4;                      // channel ranges of the host-buffer entries' pipelines
+constexpr int GENERIC_SMEM_MAX = 200 * 1024;       // the generic F kernel's largest plan (two fp32 ping-pong buffers)
+
+struct DevicePlan {
+    int pairs_f16, pairs_f16_edge, pairs_i8;       // CTA pairs the device holds at once (persistent X grids)
+};
+
+template <typename K>
+bool set_smem(K kern, int bytes)
+{
+    return cudaFuncSetAttribute(reinterpret_cast<const void *>(kern), cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess;
+}
+
+template <int N, int R1, int PTS>
+bool prep_f_pow2()
+{
+    using C = mwax::FPow2Config<N, R1, PTS>;
+    return set_smem(mwax::f_stage_pow2_kernel<N, R1, PTS, true, false, false>, C::SMEM_BYTES) &&
+           set_smem(mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, false>, C::SMEM_BYTES) &&
+           set_smem(mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, false>, C::SMEM_BYTES) &&
+           set_smem(mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, true>, C::SMEM_BYTES) &&
+           set_smem(mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, true>, C::SMEM_BYTES);
+}
+
+// CTA pairs the device can hold at once for this kernel (GPCs with an odd SM count leave one SM unpaired); 0 on error
+template <bool kInt8, bool kEdge>
+int prep_x_pair(int sm_count)
+{
+    using C = mwax::XPairConfig<kInt8, kEdge>;
+    auto kern = mwax::x_stage_pair_kernel<kInt8, kEdge>;
+    if (!set_smem(kern, C::SMEM_BYTES)) return 0;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    cfg.gridDim = dim3(2);
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = sm_count / 2;
+    return n < sm_count / 2 ? n : sm_count / 2;
+}
+
+int prepare_device(int dev, int sm_count, DevicePlan *out)
+{
+    static std::mutex mu;
+    static std::map<int, DevicePlan> done;
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = done.find(dev);
+    if (it != done.end()) { *out = it->second; return MWAX_OK; }
+    using F64 = mwax::F6400;
+    bool ok = prep_f_pow2<64, 8, 16>() && prep_f_pow2<128, 8, 16>() && prep_f_pow2<256, 16, 32>() && prep_f_pow2<512, 16, 32>() &&
+              set_smem(mwax::f_stage_6400_kernel<true, false, false>, F64::SMEM_BYTES) &&
+              set_smem(mwax::f_stage_6400_kernel<true, true, false>, F64::SMEM_BYTES) &&
+              set_smem(mwax::f_stage_6400_kernel<false, true, false>, F64::SMEM_BYTES) &&
+              set_smem(mwax::f_stage_6400_kernel<true, true, true>, F64::SMEM_BYTES) &&
+              set_smem(mwax::f_stage_6400_kernel<false, true, true>, F64::SMEM_BYTES) &&
+              set_smem(mwax::f_stage_generic_kernel, GENERIC_SMEM_MAX);
+    DevicePlan dp;
+    dp.pairs_f16 = prep_x_pair<false, false>(sm_count);
+    dp.pairs_f16_edge = prep_x_pair<false, true>(sm_count);
+    dp.pairs_i8 = prep_x_pair<true, false>(sm_count);
+    if (!ok || dp.pairs_f16 < 1 || dp.pairs_f16_edge < 1 || dp.pairs_i8 < 1) { cudaGetLastError(); return MWAX_ERR_CUDA; }
+    done[dev] = dp;
+    *out = dp;
+    return MWAX_OK;
+}
+
 // power-of-two register kernel: (N, R1, PTS) per supported length; FULL = every bin kept, SCALE = sw[] applied
 template <int N, int R1, int PTS>
 int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, bool delay, int groups, int chunks, cudaStream_t st)
 {
     using C = mwax::FPow2Config<N, R1, PTS>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        const void *kerns[5] = {(const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, true, false, false>,
-                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, false>,
-                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, false>,
-                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, true>,
-                                (const void *)mwax::f_stage_pow2_kernel<N, R1, PTS, false, true, true>};
-        for (const void *k : kerns)
-            if (cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
-                return MWAX_ERR_CUDA;
-        attr_set = true;
-    }
     dim3 grid(groups, chunks);
     if (delay) {   // the delay variants always take the (all-ones when unused) weight table
         if (full) mwax::f_stage_pow2_kernel<N, R1, PTS, true, true, true><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
@@ -159,92 +207,34 @@ int launch_f_pow2(const mwax::FParams &fp, bool full, bool scale, bool delay, in
     return MWAX_OK;
 }
 
-template <bool FULL, bool SCALE, int Q, bool DELAY = false>
-int launch_f_6400p3_q(const mwax::FParams &fp, cudaStream_t st)
+template <bool FULL, bool SCALE, bool DELAY>
+int launch_f_6400_v(const mwax::FParams &fp, int sm_count, cudaStream_t st)
 {
-    using C = mwax::F6400P3;
-    auto kern = mwax::f_stage_6400p3_kernel<FULL, SCALE, Q, DELAY>;
-    static int max_clusters = 0;
-    cudaLaunchConfig_t cfg = {};
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = Q; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    if (!max_clusters) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess)
-            return MWAX_ERR_CUDA;
-        cfg.gridDim = dim3(Q);
-        int n = 0;
-        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) return MWAX_ERR_CUDA;
-        max_clusters = n;
-    }
-    // persistent clusters; item = (frame t, group of 4 Q inputs), groups fastest
-    const long long items = (long long)((fp.n_inputs + C::G * Q - 1) / (C::G * Q)) * fp.T;
-    const int n_cl = (int)(items < max_clusters ? items : max_clusters);
-    cfg.gridDim = dim3(n_cl * Q);
-    return cudaLaunchKernelEx(&cfg, kern, fp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
+    using C = mwax::F6400;
+    // persistent CTAs, one per SM; item = (frame t, group of 8 inputs), groups fastest
+    const long long items = (long long)((fp.n_inputs + C::GI - 1) / C::GI) * fp.T;
+    const int grid = (int)(items < sm_count ? items : sm_count);
+    mwax::f_stage_6400_kernel<FULL, SCALE, DELAY><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(fp);
+    return MWAX_OK;
 }
 
-template <int Q>
-int launch_f_6400p3(const mwax::FParams &fp, bool full, bool scale, bool delay, cudaStream_t st)
+int launch_f_6400(const mwax::FParams &fp, bool full, bool scale, bool delay, int sm_count, cudaStream_t st)
 {
-    if (delay) {   // delay variants exist for the default cluster size only and always take the weight codes
-        if (full) return launch_f_6400p3_q<true, true, 2, true>(fp, st);
-        return launch_f_6400p3_q<false, true, 2, true>(fp, st);
+    if (delay) {   // the delay variants always take the weight codes / table
+        if (full) return launch_f_6400_v<true, true, true>(fp, sm_count, st);
+        return launch_f_6400_v<false, true, true>(fp, sm_count, st);
     }
-    if (full && !scale) return launch_f_6400p3_q<true, false, Q>(fp, st);
-    if (full) return launch_f_6400p3_q<true, true, Q>(fp, st);
-    return launch_f_6400p3_q<false, true, Q>(fp, st);
+    if (full && !scale) return launch_f_6400_v<true, false, false>(fp, sm_count, st);
+    if (full) return launch_f_6400_v<true, true, false>(fp, sm_count, st);
+    return launch_f_6400_v<false, true, false>(fp, sm_count, st);
 }
 
-template <bool kInt8, int BN>
-int launch_x(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::XParams &xp, int sm_count, cudaStream_t st)
-{
-    using C = mwax::XConfig<kInt8, BN>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        if (cudaFuncSetAttribute(mwax::x_stage_kernel<kInt8, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                 C::SMEM_BYTES) != cudaSuccess)
-            return MWAX_ERR_CUDA;
-        attr_set = true;
-    }
-    const int n_items = xp.n_out * xp.n_tiles;
-    if (n_items <= 0) return MWAX_OK;
-    const int grid = n_items < sm_count ? n_items : sm_count;
-    mwax::x_stage_kernel<kInt8, BN><<<grid, C::THREADS, C::SMEM_BYTES, st>>>(tmap, tmap_flat, xp);
-    return cudaGetLastError() == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
-}
-
-// CTA pairs the device can hold at once for this kernel (GPCs with an odd SM count leave one SM unpaired); 0 on error
-template <bool kInt8, bool kEdge>
-int x_pair_capacity(int sm_count)
-{
-    using C = mwax::XPairConfig<kInt8, kEdge>;
-    auto kern = mwax::x_stage_pair_kernel<kInt8, kEdge>;
-    static int max_pairs = 0;
-    if (!max_pairs) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) return 0;
-        cudaLaunchConfig_t cfg = {};
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-        cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES;
-        cfg.attrs = attr; cfg.numAttrs = 1;
-        cfg.gridDim = dim3(2);
-        int n = 0;
-        if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess || n < 1) n = sm_count / 2;
-        max_pairs = n < sm_count / 2 ? n : sm_count / 2;
-    }
-    return max_pairs;
-}
-
+// persistent grid of CTA pairs: never more pairs than run concurrently on this device (max_pairs from prepare_device)
 template <bool kInt8, bool kEdge = false>
-int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::XParams &xp, int sm_count, cudaStream_t st)
+int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const mwax::XParams &xp, int max_pairs, cudaStream_t st)
 {
     using C = mwax::XPairConfig<kInt8, kEdge>;
     auto kern = mwax::x_stage_pair_kernel<kInt8, kEdge>;
-    const int max_pairs = x_pair_capacity<kInt8, kEdge>(sm_count);
     if (max_pairs < 1) return MWAX_ERR_CUDA;
     const int n_items = (kEdge ? xp.edge_runs : xp.n_out) * xp.n_tiles;   // units of the persistent loop
     if (n_items <= 0) return MWAX_OK;
@@ -254,8 +244,7 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
     attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    int pairs = n_items < max_pairs ? n_items : max_pairs;   // persistent: never more pairs than run concurrently
-    if (const char *e = getenv("MWAX_X_PAIRS")) { const int v = atoi(e); if (v >= 1 && v < pairs) pairs = v; }
+    const int pairs = n_items < max_pairs ? n_items : max_pairs;
     cfg.gridDim = dim3(2 * pairs);
     return cudaLaunchKernelEx(&cfg, kern, tmap, tmap_flat, xp) == cudaSuccess ? MWAX_OK : MWAX_ERR_CUDA;
 }
@@ -267,13 +256,11 @@ int launch_x_pair(const CUtensorMap &tmap, const CUtensorMap &tmap_flat, const m
 // the plain schedule levels off at 0.09 ms below T = 256, the shared-edge one at 0.17 ms below T = 512).  A run of L channels
 // costs max(T, 770) + L max(F T, 860 + 770), the plain schedule max((F + 1) T, 860) per channel; the shared-edge kernel also
 // has 4 instead of 6 pipeline stages (F = 50: 3 % slower than the model says), hence the 4 % handicap and the 8 % margin.
-// MWAX_X_EDGE=0 never, =1 whenever the geometry allows it (tests); MWAX_X_EDGE_RUNS forces the run count.
-int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs)
+// `want` is MWAX_OPT_X_EDGE_RUNS: -1 = decide here (default), 0 = never, r >= 1 = r runs (at most C) whenever the geometry allows.
+int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs, int want)
 {
-    int force = -1;
-    if (const char *e = getenv("MWAX_X_EDGE")) force = atoi(e);
-    if (force == 0 || F < 2 || (F & 1) || T < 64 || pairs < 1) return 0;
-    if (const char *e = getenv("MWAX_X_EDGE_RUNS")) { const int v = atoi(e); if (v >= 1 && v <= C) return v; }
+    if (want == 0 || F < 2 || (F & 1) || T < 64 || pairs < 1) return 0;
+    if (want >= 1) return want < C ? want : C;
     const long long e_out = 860, e_add = 770;
     const long long per_chan_plain = std::max<long long>((long long)(F + 1) * T, e_out);
     const long long per_chan_edge = std::max<long long>((long long)F * T, e_out + e_add);
@@ -286,7 +273,6 @@ int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs)
         const long long cost = waves * (init + (long long)((C + r - 1) / r) * per_chan_edge);
         if (best < 0 || cost < best) { best = cost; best_r = r; }
     }
-    if (force == 1) return best_r;
     return (best * 104 <= plain * 92) ? best_r : 0;
 }
 
@@ -295,15 +281,19 @@ int choose_edge_runs(int C, int F, int T, int n_tiles, int pairs)
 // ------------------------------------------------------------------------------------------------ handles
 struct mwax_corr {
     int n, N, K, T, F, C;
+    int device;        // CUDA device the handle lives on; every call checks that it is the current one
+    DevicePlan dp;
     int avg_mode;
+    int dc_exclude;    // MWAX_OPT_DC_EXCLUDE, default 1
     int accumulate;    // MWAX_OPT_ACCUMULATE: process() adds into d_vis
-    int x_bn;          // X tile width in G columns (128 or 256)
+    int want_edge_runs;   // MWAX_OPT_X_EDGE_RUNS: -1 = auto
     int pitch;         // fp16 elements per Y row (2n rounded up to 64)
     int sm_count;
     int last_cuda;
+    long long launches;   // kernels enqueued through this handle so far
     bool tables_ready;
     // F plan
-    int f_kind;        // 0 = generic Stockham kernel, else the power-of-two register kernel for that N
+    int f_kind;        // 0 = generic Stockham kernel, else the specialised kernel for that N (64, 128, 256, 512, 6400)
     float in_scale;
     int chan_scale;
     int G;
@@ -312,14 +302,12 @@ struct mwax_corr {
     // device tables
     float2 *d_tw;
     unsigned *d_swcode;
-    int f_p3;          // N = 6400: cluster size Q (2, 4, 8) of the three-pass 20 x 20 x 16 kernel
     float *d_sw;
     int *d_tap_start;
     float *d_scale;
-    uint8_t *d_tiles;
-    uint8_t *d_ptiles;  // CTA-pair kernel's tile list
-    int n_ptiles, x_pair;
-    int n_tiles, n_taps;
+    uint8_t *d_ptiles;  // CTA-pair tile list
+    int n_ptiles;
+    int n_taps;
     int edge_runs;      // shared-edge schedule of the pair kernel: runs per tile, 0 = off, -1 = not chosen yet
     __half *d_Y;
     bool y_owned;      // false after mwax_corr_set_workspace: the caller owns the memory
@@ -337,21 +325,24 @@ struct mwax_corr {
     cudaStream_t s_in, s_out;              // copy streams of process_host
     cudaEvent_t ev_start, ev_copied;
     cudaEvent_t ev_part[8];                // channel ranges of the last dump of process_host
-    int host_tail_parts;
     std::vector<cudaEvent_t> ev_in, ev_done;
 };
 
 struct mwax_xcorr {
     int n, n_chan, n_time;
-    int x_bn;
+    int device;
+    DevicePlan dp;
     int sm_count;
     int last_cuda;
+    int pitch;          // bytes per (channel, time) row as the kernel reads it: 2n rounded up to 16 (TMA row pitch)
     int *d_tap_start;
-    uint8_t *d_tiles;
     uint8_t *d_ptiles;
-    int n_tiles, n_ptiles, x_pair;
+    int n_ptiles;
+    int8_t *d_pad;      // [chan][time][pitch] copy of a ragged (2n % 16 != 0) input, allocated on first use
     int8_t *d_in;
     int32_t *d_out;
+    cudaStream_t s_in, s_out;              // copy streams of process_host
+    cudaEvent_t ev_start, ev_in[HOST_PARTS], ev_done[HOST_PARTS], ev_copied;
 };
 
 static int note_cuda(int *slot)
@@ -367,7 +358,6 @@ static void free_tables(mwax_corr *h)
     cudaFree(h->d_swcode); h->d_swcode = nullptr;
     cudaFree(h->d_tap_start); h->d_tap_start = nullptr;
     cudaFree(h->d_scale); h->d_scale = nullptr;
-    cudaFree(h->d_tiles); h->d_tiles = nullptr;
     cudaFree(h->d_ptiles); h->d_ptiles = nullptr;
     h->tables_ready = false;
 }
@@ -402,13 +392,14 @@ static int build_tables(mwax_corr *h)
                 const int u = p - half;
                 if ((((u - F / 2) % F) + F) % F == 0) sw[p] = (float)std::sqrt(0.5);
             }
-        sw[half] = 0.0f;                                            // DC excluded (L290-294)
-        h->chan_scale = 1;
-        scale[c0] = (float)((1.0 / (s * s * F)) * (double)F / (double)(F - 1));
+        h->chan_scale = (F % 2 == 0) ? 1 : 0;
+        if (h->dc_exclude) {                                        // DC excluded, centre channel re-scaled (L290-294)
+            sw[half] = 0.0f;
+            h->chan_scale = 1;
+            scale[c0] = (float)((1.0 / (s * s * F)) * (double)F / (double)(F - 1));
+        }
     }
     std::vector<uint8_t> tiles;
-    build_tiles(h->n, h->x_bn, tiles);
-    h->n_tiles = (int)tiles.size() / 4;
     h->edge_runs = -1;
     int rc;
     if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
@@ -432,7 +423,6 @@ static int build_tables(mwax_corr *h)
     }
     if ((rc = upload(&h->d_tap_start, tap)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_scale, scale)) != MWAX_OK) return rc;
-    if ((rc = upload(&h->d_tiles, tiles)) != MWAX_OK) return rc;
     build_pair_tiles(h->n, tiles);
     h->n_ptiles = (int)tiles.size() / 4;
     if ((rc = upload(&h->d_ptiles, tiles)) != MWAX_OK) return rc;
@@ -469,15 +459,17 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
         g_last_error = MWAX_ERR_UNSUPPORTED;
         return nullptr;
     }
-    int sm = 0;
-    if ((g_last_error = check_device(&sm)) != MWAX_OK) return nullptr;
+    int sm = 0, dev = 0;
+    if ((g_last_error = check_device(&sm, &dev)) != MWAX_OK) return nullptr;
+    DevicePlan dp;
+    if ((g_last_error = prepare_device(dev, sm, &dp)) != MWAX_OK) return nullptr;
     mwax_corr *h = new (std::nothrow) mwax_corr();
     if (!h) { g_last_error = MWAX_ERR_NOMEM; return nullptr; }
     h->n = n_inputs; h->N = n_fft; h->K = n_keep; h->T = t_int; h->F = f_avg; h->C = n_keep / f_avg;
+    h->device = dev; h->dp = dp;
     h->avg_mode = MWAX_AVG_CENTRE_SYMMETRIC;
-    h->x_bn = 256;
-    if (const char *e = getenv("MWAX_X_TILE_N")) { if (atoi(e) == 128) h->x_bn = 128; }
-    h->x_pair = want_pair_kernel();
+    h->dc_exclude = 1;
+    h->want_edge_runs = -1;
     h->pitch = ((2 * n_inputs + 63) / 64) * 64;
     if ((unsigned long long)t_int * (unsigned long long)(h->pitch / 2) >= (1ull << 32)) {   // kernels keep this stride in 32 bits
         g_last_error = MWAX_ERR_UNSUPPORTED; delete h; return nullptr;
@@ -485,20 +477,16 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
     h->sm_count = sm;
     h->last_cuda = 0;
     h->radix = radix;
-    // F plan: register two-pass kernel for N in {64,128,256,512}; otherwise the generic Stockham kernel with as
+    // F plan: specialised kernels for N in {64,128,256,512,6400}; otherwise the generic Stockham kernel with as
     // many adjacent inputs per CTA as fit (two fp32 ping-pong buffers), up to 32 (128-byte segments)
     int G = 32;
-    while (G > 1 && (size_t)2 * G * n_fft * sizeof(float2) > 200 * 1024) G >>= 1;
+    while (G > 1 && (size_t)2 * G * n_fft * sizeof(float2) > (size_t)GENERIC_SMEM_MAX) G >>= 1;
     h->G = G;
     h->f_smem = (size_t)2 * G * n_fft * sizeof(float2);
     h->f_kind = 0;
-    if (const char *e = getenv("MWAX_F_GENERIC")) { if (atoi(e) == 1) n_fft = -n_fft; }
-    cudaError_t ae = cudaSuccess;
     if (n_fft == 64 || n_fft == 128 || n_fft == 256 || n_fft == 512 || n_fft == 6400) h->f_kind = n_fft;
-    // the generic kernel also serves the specialised lengths when a buffer is not 16-byte aligned
-    ae = cudaFuncSetAttribute(mwax::f_stage_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)h->f_smem);
-    if (n_fft < 0) n_fft = -n_fft;
-    if (ae != cudaSuccess) { g_last_error = MWAX_ERR_CUDA; delete h; return nullptr; }
+    // the N = 6400 kernel forms store addresses from a 32-bit byte stride between channel positions
+    if (n_fft == 6400 && (unsigned long long)t_int * (unsigned long long)(h->pitch / 2) >= (1ull << 30)) h->f_kind = 0;
     // twiddles exp(-2 pi i m / N), computed in double
     std::vector<float2> tw(n_fft);
     for (int m = 0; m < n_fft; ++m) {
@@ -506,10 +494,6 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
         tw[m] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
     }
     if ((g_last_error = upload(&h->d_tw, tw)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
-    if (h->f_kind == 6400) {
-        h->f_p3 = 2;   // cluster size of the three-pass kernel: 2 measured fastest on B200
-        if (const char *e = getenv("MWAX_F6400_Q")) { const int q = atoi(e); if (q == 2 || q == 4 || q == 8) h->f_p3 = q; }
-    }
     // workspace Y[K][T][pitch] fp16, zeroed once (pad columns stay zero)
     h->y_bytes = (size_t)n_keep * t_int * h->pitch * sizeof(__half);
     if (cudaMalloc(reinterpret_cast<void **>(&h->d_Y), h->y_bytes) != cudaSuccess) {
@@ -533,22 +517,34 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
 int mwax_corr_set_option(mwax_corr_t *h, int key, int value)
 {
     if (!h) return MWAX_ERR_NULL;
-    if (key == MWAX_OPT_AVG_MODE) {
-        if (value != MWAX_AVG_CENTRE_SYMMETRIC && value != MWAX_AVG_BLOCK) return MWAX_ERR_INVALID_ARG;
-        h->avg_mode = value;
-        return build_tables(h);
+    if (!on_device(h->device)) return MWAX_ERR_INVALID_ARG;
+    switch (key) {
+        case MWAX_OPT_AVG_MODE:
+            if (value != MWAX_AVG_CENTRE_SYMMETRIC && value != MWAX_AVG_BLOCK) return MWAX_ERR_INVALID_ARG;
+            h->avg_mode = value;
+            return build_tables(h);
+        case MWAX_OPT_DC_EXCLUDE:
+            if (value != 0 && value != 1) return MWAX_ERR_INVALID_ARG;
+            h->dc_exclude = value;
+            return build_tables(h);
+        case MWAX_OPT_ACCUMULATE:
+            if (value != 0 && value != 1) return MWAX_ERR_INVALID_ARG;
+            h->accumulate = value;
+            return MWAX_OK;
+        case MWAX_OPT_X_EDGE_RUNS:
+            if (value < -1) return MWAX_ERR_INVALID_ARG;
+            h->want_edge_runs = value;
+            h->edge_runs = -1;       // chosen again at the next call
+            return MWAX_OK;
+        default:
+            return MWAX_ERR_INVALID_ARG;
     }
-    if (key == MWAX_OPT_ACCUMULATE) {
-        if (value != 0 && value != 1) return MWAX_ERR_INVALID_ARG;
-        h->accumulate = value;
-        return MWAX_OK;
-    }
-    return MWAX_ERR_INVALID_ARG;
 }
 
 int mwax_corr_set_channel_gains(mwax_corr_t *h, const float *gain)
 {
     if (!h) return MWAX_ERR_NULL;
+    if (!on_device(h->device)) return MWAX_ERR_INVALID_ARG;
     if (!gain) {
         if (h->gains.empty()) return MWAX_OK;
         h->gains.clear();
@@ -564,7 +560,7 @@ int mwax_corr_set_channel_gains(mwax_corr_t *h, const float *gain)
 static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, int frame0, int coarse, void *stream)
 {
     if (!h || !d_volt) return MWAX_ERR_NULL;
-    if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
+    if (!h->tables_ready || !on_device(h->device)) return MWAX_ERR_INVALID_ARG;
     mwax::FParams fp;
     fp.volt = d_volt; fp.row_pitch = (long long)row_pitch; fp.sample0 = 0;
     fp.n_inputs = h->n; fp.N = h->N; fp.K = h->K; fp.T = h->T; fp.G = h->G; fp.frames_per_cta = 1;
@@ -582,8 +578,7 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
     const int f_kind = fp.vec_ok ? h->f_kind : 0;          // misaligned rows: generic kernel (scalar loads)
     if (f_kind == 6400) {
         const bool full = (h->K == h->N) && h->gains.empty(), scale = (h->chan_scale != 0) || !full;
-        int rc = h->f_p3 == 8 ? launch_f_6400p3<8>(fp, full, scale, delay, st) : h->f_p3 == 4 ? launch_f_6400p3<4>(fp, full, scale, delay, st)
-                                                                        : launch_f_6400p3<2>(fp, full, scale, delay, st);
+        int rc = launch_f_6400(fp, full, scale, delay, h->sm_count, st);
         if (rc != MWAX_OK) return rc;
     } else if (f_kind) {
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
@@ -606,6 +601,7 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
         dim3 grid((h->n + h->G - 1) / h->G, h->T);
         mwax::f_stage_generic_kernel<<<grid, 256, h->f_smem, st>>>(fp);
     }
+    ++h->launches;
     return note_cuda(&h->last_cuda);
 }
 
@@ -627,8 +623,8 @@ int mwax_corr_x_edge_runs(mwax_corr_t *h)
     if (!h) return MWAX_ERR_NULL;
     if (!h->tables_ready) return MWAX_ERR_INVALID_ARG;
     if (h->edge_runs < 0)
-        h->edge_runs = (h->x_pair && h->avg_mode == MWAX_AVG_CENTRE_SYMMETRIC && h->n_taps == h->F + 1)
-                           ? choose_edge_runs(h->C, h->F, h->T, h->n_ptiles, x_pair_capacity<false, true>(h->sm_count)) : 0;
+        h->edge_runs = (h->avg_mode == MWAX_AVG_CENTRE_SYMMETRIC && h->n_taps == h->F + 1)
+                           ? choose_edge_runs(h->C, h->F, h->T, h->n_ptiles, h->dp.pairs_f16_edge, h->want_edge_runs) : 0;
     return h->edge_runs;
 }
 
@@ -638,26 +634,19 @@ int mwax_corr_x_edge_runs(mwax_corr_t *h)
 static int x_stage_range(mwax_corr_t *h, float *d_vis, int c0, int cnt, void *stream)
 {
     if (!h || !d_vis) return MWAX_ERR_NULL;
-    if (!h->tables_ready || c0 < 0 || cnt < 1 || c0 + cnt > h->C) return MWAX_ERR_INVALID_ARG;
+    if (!h->tables_ready || c0 < 0 || cnt < 1 || c0 + cnt > h->C || !on_device(h->device)) return MWAX_ERR_INVALID_ARG;
     const bool whole = (c0 == 0 && cnt == h->C);
     mwax::XParams xp;
-    xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = cnt; xp.n_tiles = h->n_tiles;
-    xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start + c0; xp.n_taps = h->n_taps; xp.scale = h->d_scale + c0;
+    xp.n_inputs = h->n; xp.T = h->T; xp.K = h->K; xp.n_out = cnt; xp.n_tiles = h->n_ptiles;
+    xp.tiles = h->d_ptiles; xp.tap_start = h->d_tap_start + c0; xp.n_taps = h->n_taps; xp.scale = h->d_scale + c0;
     xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
     xp.out = d_vis + (size_t)c0 * (size_t)xp.out_chan_stride * 2;
     xp.accumulate = h->accumulate;
-    xp.edge_runs = 0;
-    if (h->x_pair) {
-        xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
-        xp.edge_runs = whole ? mwax_corr_x_edge_runs(h) : 0;
-        int rcp = xp.edge_runs > 0 ? launch_x_pair<false, true>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream)
-                                   : launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
-        if (rcp != MWAX_OK) note_cuda(&h->last_cuda);
-        return rcp;
-    }
-    int rc = (h->x_bn == 128) ? launch_x<false, 128>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream)
-                              : launch_x<false, 256>(h->tmap, h->tmap_flat, xp, h->sm_count, (cudaStream_t)stream);
+    xp.edge_runs = whole ? mwax_corr_x_edge_runs(h) : 0;
+    int rc = xp.edge_runs > 0 ? launch_x_pair<false, true>(h->tmap, h->tmap_flat, xp, h->dp.pairs_f16_edge, (cudaStream_t)stream)
+                              : launch_x_pair<false>(h->tmap, h->tmap_flat, xp, h->dp.pairs_f16, (cudaStream_t)stream);
     if (rc != MWAX_OK) note_cuda(&h->last_cuda);
+    else ++h->launches;
     return rc;
 }
 
@@ -672,11 +661,11 @@ int mwax_corr_process_batch(mwax_corr_t *h, const int8_t *d_volt, size_t row_pit
 {
     if (!h || !d_volt || !d_vis) return MWAX_ERR_NULL;
     if (n_dumps < 1 || n_coarse < 1 || row_pitch < (size_t)n_dumps * h->T * h->N) return MWAX_ERR_INVALID_ARG;
+    if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)n_dumps * h->T) return MWAX_ERR_INVALID_ARG;
     const size_t dump_samples = (size_t)h->T * h->N;
     const size_t vis_floats = (size_t)h->C * ((size_t)h->n * (h->n + 1) / 2) * 2;
     for (int c = 0; c < n_coarse; ++c)
         for (int d = 0; d < n_dumps; ++d) {
-            if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)(d + 1) * h->T) return MWAX_ERR_INVALID_ARG;
             int rc = f_stage_impl(h, d_volt + 2 * (c * coarse_pitch + d * dump_samples), row_pitch, d * h->T, c, stream);
             if (rc != MWAX_OK) return rc;
             rc = mwax_corr_x_stage(h, d_vis + ((size_t)c * n_dumps + d) * vis_floats, stream);
@@ -695,7 +684,12 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
                            int n_coarse, float *h_vis, void *stream)
 {
     if (!h || !h_volt || !h_vis) return MWAX_ERR_NULL;
-    if (n_dumps < 1 || n_coarse < 1 || row_pitch < (size_t)n_dumps * h->T * h->N) return MWAX_ERR_INVALID_ARG;
+    // every argument check comes before the first enqueue; with MWAX_OPT_ACCUMULATE the sum would go into the staging
+    // buffer, not into h_vis: refused rather than silently wrong
+    if (n_dumps < 1 || n_coarse < 1 || row_pitch < (size_t)n_dumps * h->T * h->N || h->accumulate || !h->tables_ready ||
+        !on_device(h->device))
+        return MWAX_ERR_INVALID_ARG;
+    if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)n_dumps * h->T) return MWAX_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     const size_t dump_samples = (size_t)h->T * h->N;
     const size_t row_samples = (size_t)n_dumps * dump_samples;
@@ -704,12 +698,12 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
     const size_t out_bytes = (size_t)n_dumps * dump_out;
     if (h->in_bytes < in_bytes) {
         cudaFree(h->d_in); h->d_in = nullptr; h->in_bytes = 0;
-        if (cudaMalloc(reinterpret_cast<void **>(&h->d_in), in_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
+        if (cudaMalloc(reinterpret_cast<void **>(&h->d_in), in_bytes) != cudaSuccess) { cudaGetLastError(); return MWAX_ERR_NOMEM; }
         h->in_bytes = in_bytes;
     }
     if (h->out_bytes < out_bytes) {
         cudaFree(h->d_out); h->d_out = nullptr; h->out_bytes = 0;
-        if (cudaMalloc(reinterpret_cast<void **>(&h->d_out), out_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
+        if (cudaMalloc(reinterpret_cast<void **>(&h->d_out), out_bytes) != cudaSuccess) { cudaGetLastError(); return MWAX_ERR_NOMEM; }
         h->out_bytes = out_bytes;
     }
     // Three streams so that PCIe runs in both directions under the kernels: dump d + 1 travels host -> device and
@@ -731,9 +725,15 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
             return note_cuda(&h->last_cuda);
         for (int q = 0; q < 8; ++q)
             if (cudaEventCreateWithFlags(&h->ev_part[q], cudaEventDisableTiming) != cudaSuccess) return note_cuda(&h->last_cuda);
-        h->host_tail_parts = 4;
-        if (const char *pe = getenv("MWAX_HOST_TAIL_PARTS")) { const int v = atoi(pe); if (v >= 1 && v <= 8) h->host_tail_parts = v; }
     }
+    // once work is in flight an error must not return while copies still reference the caller's host buffers
+    auto fail = [&](int rc) {
+        cudaStreamSynchronize(h->s_in);
+        cudaStreamSynchronize(h->s_out);
+        cudaStreamSynchronize(st);
+        if (rc == MWAX_ERR_CUDA) note_cuda(&h->last_cuda);
+        return rc;
+    };
     // the copy streams start after whatever the caller has already queued on `stream`
     cudaEventRecord(h->ev_start, st);
     cudaStreamWaitEvent(h->s_in, h->ev_start, 0);
@@ -747,28 +747,27 @@ int mwax_corr_process_host(mwax_corr_t *h, const int8_t *h_volt, size_t row_pitc
             if (cudaMemcpy2DAsync(h->d_in + 2 * d * dump_samples, row_samples * 2,
                                   h_volt + 2 * (c * coarse_pitch + d * dump_samples), row_pitch * 2, dump_samples * 2, h->n,
                                   cudaMemcpyHostToDevice, h->s_in) != cudaSuccess)
-                return note_cuda(&h->last_cuda);
+                return fail(MWAX_ERR_CUDA);
             cudaEventRecord(h->ev_in[e], h->s_in);
             cudaStreamWaitEvent(st, h->ev_in[e], 0);
             if (c > 0) cudaStreamWaitEvent(st, h->ev_copied, 0);   // previous channel's visibilities have left d_out
-            if ((h->d_delay || h->d_phase) && h->d_row_stride < (size_t)(d + 1) * h->T) return MWAX_ERR_INVALID_ARG;
             int rc = f_stage_impl(h, h->d_in + 2 * d * dump_samples, row_samples, d * h->T, c, st);
-            if (rc != MWAX_OK) return rc;
-            // Nothing hides the device -> host copy of the LAST dump: it is correlated in `parts` channel ranges and each
+            if (rc != MWAX_OK) return fail(rc);
+            // Nothing hides the device -> host copy of the LAST dump: it is correlated in HOST_PARTS channel ranges and each
             // range leaves while the next is computed (plain schedule only; earlier dumps travel under the next dump's work).
             int parts = 1;
-            if (e == n_ev - 1 && !h->accumulate && h->C >= 8 && !(h->x_pair && mwax_corr_x_edge_runs(h) > 0)) parts = h->host_tail_parts;
+            if (e == n_ev - 1 && h->C >= 8 && mwax_corr_x_edge_runs(h) <= 0) parts = HOST_PARTS;
             for (int q = 0; q < parts; ++q) {
                 const int c0 = (int)(((long long)q * h->C) / parts), c1 = (int)(((long long)(q + 1) * h->C) / parts);
                 rc = x_stage_range(h, h->d_out + (size_t)d * vis_floats, c0, c1 - c0, st);
-                if (rc != MWAX_OK) return rc;
+                if (rc != MWAX_OK) return fail(rc);
                 cudaEventRecord(q == parts - 1 ? h->ev_done[e] : h->ev_part[q], st);
                 cudaStreamWaitEvent(h->s_out, q == parts - 1 ? h->ev_done[e] : h->ev_part[q], 0);
                 const size_t off = (size_t)c0 * (dump_out / h->C), len = (size_t)(c1 - c0) * (dump_out / h->C);
                 if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c * out_bytes + (size_t)d * dump_out + off,
                                     reinterpret_cast<char *>(h->d_out + (size_t)d * vis_floats) + off, len, cudaMemcpyDeviceToHost,
                                     h->s_out) != cudaSuccess)
-                    return note_cuda(&h->last_cuda);
+                    return fail(MWAX_ERR_CUDA);
             }
             if (d == n_dumps - 1) cudaEventRecord(h->ev_copied, h->s_out);
         }
@@ -788,13 +787,17 @@ int mwax_corr_set_workspace(mwax_corr_t *h, void *d_ws, size_t bytes)
 {
     if (!h || !d_ws) return MWAX_ERR_NULL;
     if (bytes < h->y_bytes || (reinterpret_cast<uintptr_t>(d_ws) & 255u)) return MWAX_ERR_INVALID_ARG;
+    if (!on_device(h->device)) return MWAX_ERR_INVALID_ARG;
     if (cudaMemset(d_ws, 0, h->y_bytes) != cudaSuccess) return note_cuda(&h->last_cuda);   // pad columns must read as zero
-    int rc = encode_z_map(&h->tmap, false, d_ws, (uint64_t)h->pitch, (uint64_t)h->pitch * 2, (uint64_t)h->T, (uint64_t)h->K, 64);
+    CUtensorMap m1, m2;      // both maps are encoded before anything in the handle changes
+    int rc = encode_z_map(&m1, false, d_ws, (uint64_t)h->pitch, (uint64_t)h->pitch * 2, (uint64_t)h->T, (uint64_t)h->K, 64);
     if (rc == MWAX_OK)
-        rc = encode_z_map(&h->tmap_flat, false, d_ws, (uint64_t)h->pitch, (uint64_t)h->pitch * 2, (uint64_t)h->T * h->K, 1, 64);
+        rc = encode_z_map(&m2, false, d_ws, (uint64_t)h->pitch, (uint64_t)h->pitch * 2, (uint64_t)h->T * h->K, 1, 64);
     if (rc != MWAX_OK) return rc;
     if (cudaDeviceSynchronize() != cudaSuccess) return note_cuda(&h->last_cuda);
     if (h->y_owned) cudaFree(h->d_Y);
+    h->tmap = m1;
+    h->tmap_flat = m2;
     h->d_Y = reinterpret_cast<__half *>(d_ws);
     h->y_owned = false;
     return MWAX_OK;
@@ -818,6 +821,7 @@ int mwax_corr_to_mwax_order_weighted(mwax_corr_t *h, const float *d_vis, const u
     if (!h || !d_vis || !d_out) return MWAX_ERR_NULL;
     if (d_flags && n_sub < 1) return MWAX_ERR_INVALID_ARG;
     if (h->n & 1) return MWAX_ERR_UNSUPPORTED;              // tiles are pairs of signal paths (x, y)
+    if (!on_device(h->device)) return MWAX_ERR_INVALID_ARG;
     mwax::OrderParams op;
     op.vis = reinterpret_cast<const float2 *>(d_vis); op.out = reinterpret_cast<float2 *>(d_out); op.weights = d_weights;
     op.n_tiles = h->n / 2; op.C = h->C; op.chan_stride = (long long)h->n * (h->n + 1) / 2;
@@ -825,11 +829,12 @@ int mwax_corr_to_mwax_order_weighted(mwax_corr_t *h, const float *d_vis, const u
     dim3 grid((op.n_tiles + mwax::ORD_TA - 1) / mwax::ORD_TA, op.n_tiles, (op.C + mwax::ORD_TC - 1) / mwax::ORD_TC);
     if (grid.y > 65535 || grid.z > 65535) return MWAX_ERR_UNSUPPORTED;
     mwax::mwax_order_kernel<<<grid, 256, 0, (cudaStream_t)stream>>>(op);
+    ++h->launches;
     return note_cuda(&h->last_cuda);
 }
 
 size_t mwax_corr_workspace_bytes(const mwax_corr_t *h) { return h ? h->y_bytes : 0; }
-int mwax_corr_launches_per_process(const mwax_corr_t *h) { return h ? 2 : 0; }
+long long mwax_corr_launch_count(const mwax_corr_t *h) { return h ? h->launches : 0; }
 int mwax_corr_last_cuda_error(const mwax_corr_t *h) { return h ? h->last_cuda : 0; }
 
 int mwax_corr_destroy(mwax_corr_t *h)
@@ -856,69 +861,118 @@ mwax_xcorr_t *mwax_xcorr_i8_create(int n_inputs, int n_chan, int n_time)
 {
     g_last_error = MWAX_OK;
     if (n_inputs < 1 || n_chan < 1 || n_time < 1) { g_last_error = MWAX_ERR_INVALID_ARG; return nullptr; }
-    if (n_inputs % 8 != 0 || n_inputs > 8128 || n_time > 65535) { g_last_error = MWAX_ERR_UNSUPPORTED; return nullptr; }
-    int sm = 0;
-    if ((g_last_error = check_device(&sm)) != MWAX_OK) return nullptr;
+    if (n_inputs > 8128 || n_time > 65535) { g_last_error = MWAX_ERR_UNSUPPORTED; return nullptr; }
+    int sm = 0, dev = 0;
+    if ((g_last_error = check_device(&sm, &dev)) != MWAX_OK) return nullptr;
+    DevicePlan dp;
+    if ((g_last_error = prepare_device(dev, sm, &dp)) != MWAX_OK) return nullptr;
     mwax_xcorr *h = new (std::nothrow) mwax_xcorr();
     if (!h) { g_last_error = MWAX_ERR_NOMEM; return nullptr; }
     h->n = n_inputs; h->n_chan = n_chan; h->n_time = n_time; h->sm_count = sm; h->last_cuda = 0;
-    h->x_bn = 256;
-    if (const char *e = getenv("MWAX_X_TILE_N")) { if (atoi(e) == 128) h->x_bn = 128; }
+    h->device = dev; h->dp = dp;
+    h->pitch = ((2 * n_inputs + 15) / 16) * 16;
     std::vector<int> tap(n_chan);
     for (int c = 0; c < n_chan; ++c) tap[c] = c;
-    std::vector<uint8_t> tiles;
-    build_tiles(n_inputs, h->x_bn, tiles);
-    h->n_tiles = (int)tiles.size() / 4;
     std::vector<uint8_t> ptiles;
     build_pair_tiles(n_inputs, ptiles);
     h->n_ptiles = (int)ptiles.size() / 4;
-    h->x_pair = want_pair_kernel();
     if ((g_last_error = upload(&h->d_tap_start, tap)) != MWAX_OK ||
-        (g_last_error = upload(&h->d_ptiles, ptiles)) != MWAX_OK ||
-        (g_last_error = upload(&h->d_tiles, tiles)) != MWAX_OK) {
+        (g_last_error = upload(&h->d_ptiles, ptiles)) != MWAX_OK) {
         mwax_xcorr_i8_destroy(h); return nullptr;
     }
     return h;
 }
 
+// channels [c0, c0 + cnt) of a resident buffer `d_z` with row pitch `pitch` bytes (a multiple of 16, base 16-byte aligned)
+static int xcorr_i8_range(mwax_xcorr_t *h, const int8_t *d_z, int pitch, int32_t *d_vis, int c0, int cnt, cudaStream_t st)
+{
+    CUtensorMap tmap;   // columns past 2n read as zero (TMA out-of-bounds fill): that pads partial tiles and ragged rows
+    int rc = encode_z_map(&tmap, true, d_z, (uint64_t)2 * h->n, (uint64_t)pitch, (uint64_t)h->n_time, (uint64_t)h->n_chan, 128);
+    if (rc != MWAX_OK) return rc;
+    mwax::XParams xp;
+    xp.n_inputs = h->n; xp.T = h->n_time; xp.K = h->n_chan; xp.n_out = cnt; xp.n_tiles = h->n_ptiles;
+    xp.tiles = h->d_ptiles; xp.tap_start = h->d_tap_start + c0; xp.n_taps = 1; xp.scale = nullptr;
+    xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
+    xp.out = d_vis + (size_t)c0 * (size_t)xp.out_chan_stride * 2;
+    xp.accumulate = 0;
+    xp.edge_runs = 0;
+    rc = launch_x_pair<true>(tmap, tmap, xp, h->dp.pairs_i8, st);
+    if (rc != MWAX_OK) note_cuda(&h->last_cuda);
+    return rc;
+}
+
 int mwax_xcorr_i8_process(mwax_xcorr_t *h, const int8_t *d_z, int32_t *d_vis, void *stream)
 {
     if (!h || !d_z || !d_vis) return MWAX_ERR_NULL;
-    if (reinterpret_cast<uintptr_t>(d_z) & 15u) return MWAX_ERR_INVALID_ARG;
-    CUtensorMap tmap;
-    int rc = encode_z_map(&tmap, true, d_z, (uint64_t)2 * h->n, (uint64_t)2 * h->n, (uint64_t)h->n_time,
-                          (uint64_t)h->n_chan, 128);
-    if (rc != MWAX_OK) return rc;
-    mwax::XParams xp;
-    xp.n_inputs = h->n; xp.T = h->n_time; xp.K = h->n_chan; xp.n_out = h->n_chan; xp.n_tiles = h->n_tiles;
-    xp.tiles = h->d_tiles; xp.tap_start = h->d_tap_start; xp.n_taps = 1; xp.scale = nullptr;
-    xp.out = d_vis; xp.out_chan_stride = (long long)h->n * (h->n + 1) / 2;
-    xp.accumulate = 0;
-    xp.edge_runs = 0;
-    if (h->x_pair) {
-        xp.n_tiles = h->n_ptiles; xp.tiles = h->d_ptiles;
-        rc = launch_x_pair<true>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream);
-        if (rc != MWAX_OK) note_cuda(&h->last_cuda);
-        return rc;
+    if (!on_device(h->device)) return MWAX_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool direct = (h->pitch == 2 * h->n) && ((reinterpret_cast<uintptr_t>(d_z) & 15u) == 0);
+    if (direct) return xcorr_i8_range(h, d_z, h->pitch, d_vis, 0, h->n_chan, st);
+    // TMA needs a 16-byte aligned base and row pitch: a ragged (n_inputs % 8 != 0) or misaligned buffer is first copied,
+    // on the device, into rows of the next multiple of 16 bytes (one extra pass over the input; the pad bytes are never
+    // used: the tensor map's inner extent stays 2n)
+    const size_t rows = (size_t)h->n_chan * h->n_time;
+    if (!h->d_pad && cudaMalloc(reinterpret_cast<void **>(&h->d_pad), rows * (size_t)h->pitch) != cudaSuccess) {
+        cudaGetLastError();
+        return MWAX_ERR_NOMEM;
     }
-    rc = (h->x_bn == 128) ? launch_x<true, 128>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream)
-                          : launch_x<true, 256>(tmap, tmap, xp, h->sm_count, (cudaStream_t)stream);
-    if (rc != MWAX_OK) note_cuda(&h->last_cuda);
-    return rc;
+    if (cudaMemcpy2DAsync(h->d_pad, (size_t)h->pitch, d_z, (size_t)2 * h->n, (size_t)2 * h->n, rows, cudaMemcpyDeviceToDevice, st) !=
+        cudaSuccess)
+        return note_cuda(&h->last_cuda);
+    return xcorr_i8_range(h, h->d_pad, h->pitch, d_vis, 0, h->n_chan, st);
 }
 
 int mwax_xcorr_i8_process_host(mwax_xcorr_t *h, const int8_t *h_z, int32_t *h_vis, void *stream)
 {
     if (!h || !h_z || !h_vis) return MWAX_ERR_NULL;
+    if (!on_device(h->device)) return MWAX_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
-    const size_t in_bytes = (size_t)h->n_chan * h->n_time * h->n * 2;
-    const size_t out_bytes = (size_t)h->n_chan * ((size_t)h->n * (h->n + 1) / 2) * 8;
-    if (!h->d_in && cudaMalloc(reinterpret_cast<void **>(&h->d_in), in_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
-    if (!h->d_out && cudaMalloc(reinterpret_cast<void **>(&h->d_out), out_bytes) != cudaSuccess) return MWAX_ERR_NOMEM;
-    if (cudaMemcpyAsync(h->d_in, h_z, in_bytes, cudaMemcpyHostToDevice, st) != cudaSuccess) return note_cuda(&h->last_cuda);
-    int rc = mwax_xcorr_i8_process(h, h->d_in, h->d_out, st);
-    if (rc != MWAX_OK) return rc;
-    if (cudaMemcpyAsync(h_vis, h->d_out, out_bytes, cudaMemcpyDeviceToHost, st) != cudaSuccess) return note_cuda(&h->last_cuda);
+    const size_t rows = (size_t)h->n_chan * h->n_time;
+    const size_t chan_out = ((size_t)h->n * (h->n + 1) / 2) * 8;
+    if (!h->d_in && cudaMalloc(reinterpret_cast<void **>(&h->d_in), rows * (size_t)h->pitch) != cudaSuccess) { cudaGetLastError(); return MWAX_ERR_NOMEM; }
+    if (!h->d_out && cudaMalloc(reinterpret_cast<void **>(&h->d_out), (size_t)h->n_chan * chan_out) != cudaSuccess) { cudaGetLastError(); return MWAX_ERR_NOMEM; }
+    if (!h->s_in) {
+        if (cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->ev_start, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&h->ev_copied, cudaEventDisableTiming) != cudaSuccess)
+            return note_cuda(&h->last_cuda);
+        for (int q = 0; q < HOST_PARTS; ++q)
+            if (cudaEventCreateWithFlags(&h->ev_in[q], cudaEventDisableTiming) != cudaSuccess ||
+                cudaEventCreateWithFlags(&h->ev_done[q], cudaEventDisableTiming) != cudaSuccess)
+                return note_cuda(&h->last_cuda);
+    }
+    auto fail = [&](int rc) {
+        cudaStreamSynchronize(h->s_in);
+        cudaStreamSynchronize(h->s_out);
+        cudaStreamSynchronize(st);
+        if (rc == MWAX_ERR_CUDA) note_cuda(&h->last_cuda);
+        return rc;
+    };
+    // channels are independent: range q + 1 travels host -> device and range q - 1 device -> host while range q is
+    // correlated (the host rows are copied straight into 16-byte pitched rows, so any n_inputs costs no extra pass here)
+    cudaEventRecord(h->ev_start, st);
+    cudaStreamWaitEvent(h->s_in, h->ev_start, 0);
+    cudaStreamWaitEvent(h->s_out, h->ev_start, 0);
+    const int parts = h->n_chan >= HOST_PARTS ? HOST_PARTS : 1;
+    for (int q = 0; q < parts; ++q) {
+        const int c0 = (int)(((long long)q * h->n_chan) / parts), c1 = (int)(((long long)(q + 1) * h->n_chan) / parts);
+        const size_t r0 = (size_t)c0 * h->n_time, nr = (size_t)(c1 - c0) * h->n_time;
+        if (cudaMemcpy2DAsync(h->d_in + r0 * (size_t)h->pitch, (size_t)h->pitch, h_z + r0 * (size_t)2 * h->n, (size_t)2 * h->n,
+                              (size_t)2 * h->n, nr, cudaMemcpyHostToDevice, h->s_in) != cudaSuccess)
+            return fail(MWAX_ERR_CUDA);
+        cudaEventRecord(h->ev_in[q], h->s_in);
+        cudaStreamWaitEvent(st, h->ev_in[q], 0);
+        int rc = xcorr_i8_range(h, h->d_in, h->pitch, h->d_out, c0, c1 - c0, st);
+        if (rc != MWAX_OK) return fail(rc);
+        cudaEventRecord(h->ev_done[q], st);
+        cudaStreamWaitEvent(h->s_out, h->ev_done[q], 0);
+        if (cudaMemcpyAsync(reinterpret_cast<char *>(h_vis) + (size_t)c0 * chan_out, reinterpret_cast<char *>(h->d_out) + (size_t)c0 * chan_out,
+                            (size_t)(c1 - c0) * chan_out, cudaMemcpyDeviceToHost, h->s_out) != cudaSuccess)
+            return fail(MWAX_ERR_CUDA);
+    }
+    cudaEventRecord(h->ev_copied, h->s_out);
+    cudaStreamWaitEvent(st, h->ev_copied, 0);
     if (cudaStreamSynchronize(st) != cudaSuccess) return note_cuda(&h->last_cuda);
     return MWAX_OK;
 }
@@ -927,10 +981,18 @@ int mwax_xcorr_i8_destroy(mwax_xcorr_t *h)
 {
     if (!h) return MWAX_OK;
     cudaFree(h->d_tap_start);
-    cudaFree(h->d_tiles);
     cudaFree(h->d_ptiles);
+    cudaFree(h->d_pad);
     cudaFree(h->d_in);
     cudaFree(h->d_out);
+    if (h->s_in) cudaStreamDestroy(h->s_in);
+    if (h->s_out) cudaStreamDestroy(h->s_out);
+    if (h->ev_start) cudaEventDestroy(h->ev_start);
+    if (h->ev_copied) cudaEventDestroy(h->ev_copied);
+    for (int q = 0; q < HOST_PARTS; ++q) {
+        if (h->ev_in[q]) cudaEventDestroy(h->ev_in[q]);
+        if (h->ev_done[q]) cudaEventDestroy(h->ev_done[q]);
+    }
     delete h;
     return MWAX_OK;
 }

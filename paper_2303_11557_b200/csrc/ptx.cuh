@@ -18,10 +18,6 @@ __device__ __forceinline__ void fence_mbar_init()
 {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar)
-{
-    asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.shared::cta.b64 st, [%0];\n}" ::"r"(bar) : "memory");
-}
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
 {
     asm volatile("{\n .reg .b64 st;\n mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n}" ::"r"(bar), "r"(bytes)
@@ -37,13 +33,26 @@ __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t bar, uint32_t parity)
         : "memory");
     return ok;
 }
-// Spin with a watchdog: a protocol bug must trap (-> cudaErrorLaunchFailure) instead of hanging the GPU.
+// Wait on an mbarrier phase.  try_wait suspends the thread in hardware for a bounded time, so the loop is not a busy
+// spin.  The watchdog is WALL-CLOCK based (%globaltimer, checked every 4096 polls): a healthy wait of any length that a
+// long integration, a profiler replay or time slicing can produce passes, while a protocol bug still ends in a trap
+// (-> cudaErrorLaunchFailure) after 20 s instead of hanging the GPU for ever.  -DMWAX_NO_WATCHDOG removes it.
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
 {
-    uint32_t spins = 0;
+#ifdef MWAX_NO_WATCHDOG
+    while (!mbar_try_wait(bar, parity)) {}
+#else
+    uint32_t polls = 0;
+    unsigned long long t0 = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > (1u << 24)) __trap();
+        if ((++polls & 4095u) == 0) {
+            unsigned long long now;
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(now));
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 20000000000ull) __trap();
+        }
     }
+#endif
 }
 
 // ---------------------------------------------------------------- TMA
@@ -51,15 +60,6 @@ __device__ __forceinline__ void prefetch_tensormap(const CUtensorMap *m)
 {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(m)) : "memory");
 }
-// 3-D tiled load global -> shared, completion signalled on an mbarrier (complete_tx::bytes)
-__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap *m, int c0, int c1, int c2, uint32_t bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
-        ::"r"(dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(c0), "r"(c1), "r"(c2), "r"(bar)
-        : "memory");
-}
-
 // ---------------------------------------------------------------- tcgen05
 __device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols)
 {
@@ -76,12 +76,6 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols)
 }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-
-// tcgen05.commit: the mbarrier receives one arrival when all prior tcgen05.mma of this thread have completed
-__device__ __forceinline__ void tc_commit(uint32_t bar)
-{
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
-}
 
 // TMEM -> registers: this warp's 32 lanes x 32 consecutive 32-bit columns (thread L gets lane base+L)
 __device__ __forceinline__ void tmem_ld_32x32b_x32(uint32_t taddr, uint32_t (&r)[32])
@@ -117,21 +111,7 @@ __device__ __forceinline__ uint32_t mapa(uint32_t saddr, uint32_t rank)
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank));
     return r;
 }
-// arrive on an mbarrier anywhere in the cluster (address from mapa)
-// generic-proxy writes to shared memory -> visible to the async proxy (bulk copies that read them)
-__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-// bulk copy of `bytes` (multiple of 16, both addresses 16-byte aligned) from this CTA's shared memory to the shared
-// memory of another CTA of the cluster; completion is counted in bytes on `cluster_bar`, an mbarrier of the destination CTA
-__device__ __forceinline__ void bulk_copy_to_cluster(uint32_t cluster_dst, uint32_t src, uint32_t bytes, uint32_t cluster_bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 :: "r"(cluster_dst), "r"(src), "r"(bytes), "r"(cluster_bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar)
-{
-    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
-}
-// The same without release semantics.  `.release.cluster` compiles to MEMBAR.ALL.GPU + ERRBAR in front of the arrive, i.e. it
+// Arrive on an mbarrier anywhere in the cluster (address from mapa), WITHOUT release semantics: `.release.cluster` compiles to MEMBAR.ALL.GPU + ERRBAR in front of the arrive, i.e. it
 // waits until every global store the thread has issued is acknowledged: for an epilogue warp handing its TMEM accumulator
 // back that is its whole output tile (ncu, short integrations: 19 % of the epilogue's stall samples on that ERRBAR).  What
 // the hand-over must order is the TMEM reads, and those are complete once tcgen05.wait::ld has returned.

@@ -1,5 +1,8 @@
-// x_stage2.cuh — X stage on CTA PAIRS: the same contraction, schedule and epilogue as x_stage.cuh, with
-// tcgen05 cta_group::2 instructions so that two SMs work on one 256 x 256 tile of G.
+// x_stage2.cuh — the X-stage kernel: persistent CTA PAIRS (tcgen05 cta_group::2), two SMs on one 256 x 256 tile of G.
+// 6 warps per CTA: warp 0 = TMA producer (one lane), warp 1 = MMA issuer (+ TMEM owner; all lanes run the loops, one
+// elected lane issues), warps 2..5 = epilogue (TMEM lanes 32*(warp%4)..+31).  A work item is (output channel c, G-tile);
+// the 128 x 256 accumulator per CTA is double buffered in TMEM so the epilogue of one item overlaps the MMAs of the
+// next.  Work items are ordered channel-major so concurrently running pairs share a channel's rows in L2.
 //
 // Why: ncu on the single-CTA kernel (128 x 256 tiles) shows ~12 TB/s of L2 -> SM operand traffic (253 M sectors in
 // 0.68 ms at C3), i.e. the kernel sits on the L2 bandwidth limit, not on the tensor pipe (profiles/r1_ncu_full.md);
@@ -95,7 +98,13 @@ __global__ void __launch_bounds__(192, 1) x_stage_pair_kernel(const __grid_const
 
     const int n_items = P.n_out * P.n_tiles;
     const int kb_per_tap = (P.T + C::BK - 1) / C::BK;
-    const bool flat = (P.n_taps > 1) && (P.T >= C::BK);    // see x_stage.cuh: whole-block K loop over adjacent taps
+    // K-loop schedule of one work item (identical in the producer and the MMA issuer).  The taps of an output channel
+    // are adjacent channel positions, i.e. ADJACENT ROWS of Y[p][t]: when T >= BK the contraction runs over the flattened
+    // rows (p T + t) in whole BK-row blocks through `tmap_flat`, so only the END of a run is a partial block (C4: 51 taps
+    // x 200 rows = 159 blocks + 24 rows instead of 51 x (3 blocks + 8 rows)).  The partial block is fetched through the
+    // per-channel map, whose rows past T read as zero.  A tap window that wraps past K (cyclic taps, Q8) is
+    // two runs.
+    const bool flat = (P.n_taps > 1) && (P.T >= C::BK);
 
     // kEdge: the work of this pair, identical in the three roles.  Unit = (run r of adjacent output channels, tile);
     // fn(c, tile, first tap position, taps, mode) once per accumulator (x_stage.cuh, X_EDGE_*)

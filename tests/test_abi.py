@@ -47,9 +47,20 @@ def test_argument_validation_is_synchronous_and_needs_no_gpu():
     assert not L.mwax_corr_create(16, 12800, 64, 1, 1) and L.mwax_corr_last_error() == -3   # > 6400
     assert not L.mwax_corr_create(16, 64, 128, 1, 1) and L.mwax_corr_last_error() == -3     # keep > fft
     assert not L.mwax_corr_create(16, 64, 64, 1, 3) and L.mwax_corr_last_error() == -3      # 3 does not divide 64
-    assert not L.mwax_xcorr_i8_create(12, 4, 100) and L.mwax_corr_last_error() == -3        # n % 8 != 0
+    assert not L.mwax_xcorr_i8_create(12, 4, 70000) and L.mwax_corr_last_error() == -3      # int32 could overflow
+    assert not L.mwax_xcorr_i8_create(0, 4, 100) and L.mwax_corr_last_error() == -2
     assert L.mwax_corr_destroy(None) == 0 and L.mwax_xcorr_i8_destroy(None) == 0
     assert L.mwax_corr_process(None, None, None, None) == -1
+
+
+def test_library_reads_no_environment_variables():
+    """Every knob is an argument or a set_option key (include/mwax_corr.h): no getenv in the product sources."""
+    csrc = os.path.join(ROOT, "paper_2303_11557_b200", "csrc")
+    for f in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, f)).read(), f"{f} reads the environment"
+    hdr = open(HEADER).read()
+    for opt in ("MWAX_OPT_AVG_MODE", "MWAX_OPT_ACCUMULATE", "MWAX_OPT_DC_EXCLUDE", "MWAX_OPT_X_EDGE_RUNS"):
+        assert opt in hdr and hasattr(corr, opt)
 
 
 def test_product_path_fails_loudly_without_a_device():

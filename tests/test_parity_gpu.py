@@ -43,8 +43,10 @@ def _gather_sel(full, sel):
     return full[..., idx]
 
 
-def _run_fx(volt, n, N, K, T, F, mode=0, n_dumps=1):
+def _run_fx(volt, n, N, K, T, F, mode=0, n_dumps=1, options=()):
     h = corr.MwaxCorr(n, N, K, T, F, avg_mode=mode)
+    for key, value in options:
+        h.set_option(key, value)
     v = torch.from_numpy(volt).cuda()
     out = h.new_output(n_dumps=n_dumps)
     out.fill_(float("nan"))
@@ -186,6 +188,51 @@ def test_fx_full_scale_tone_does_not_overflow_fp16():
     assert _norm_err(got, ref, n) <= TOL
 
 
+@pytest.mark.parametrize("n,N,K,T,F", [
+    (40, 128, 128, 6, 1),       # register kernel, N = 128, every bin kept
+    (40, 256, 256, 5, 2),       # register kernel, N = 256, FULL + SCALE variant
+    (40, 256, 200, 5, 4),       # register kernel, N = 256, keep < fft
+    (40, 64, 64, 7, 1),         # register kernel, N = 64
+    (12, 100, 100, 6, 5),       # generic Stockham kernel
+    (12, 6400, 6400, 2, 50),    # N = 6400 kernel (byte-permute promotion since round 2)
+])
+def test_fx_minus_128_and_plus_127_samples(n, N, K, T, F):
+    """-128 is a legal sample (reading Q9) that the seeded generator never makes (it clips to +-127): rows of nothing but
+    {-128, +127}, a row that is -128 seven times out of ten and an alternating row with random flips go through every F
+    kernel's int8 -> fp32 promotion.  (Exactly constant or exactly alternating rows would have exactly-zero channels,
+    where the normalised error is 0/0.)"""
+    rng = np.random.default_rng(128 + N)
+    volt = synth.gauss_voltages(synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[], seed=128 + n + N))
+    volt[1] = rng.choice(np.array([-128, 127], dtype=np.int8), size=(N * T, 2))
+    volt[2] = np.where(rng.random((N * T, 2)) < 0.7, -128, rng.integers(-128, 128, size=(N * T, 2))).astype(np.int8)
+    alt = np.where(np.arange(N * T)[:, None] % 2 == 0, -128, 127) * np.where(rng.random((N * T, 2)) < 0.1, 0, 1)
+    volt[5] = alt.astype(np.int8)
+    volt[n - 1] = rng.choice(np.array([-128, -127, 0, 127], dtype=np.int8), size=(N * T, 2))
+    ref = oracle.fx(volt, N, K, T, F)
+    got = _run_fx(volt, n, N, K, T, F)[0]
+    assert np.isfinite(got.view(np.float64)).all()
+    assert _norm_err(got, ref, n) <= TOL
+
+
+@pytest.mark.parametrize("n,N,K,T,F", [(16, 64, 64, 40, 4), (20, 128, 96, 9, 3), (10, 6400, 6400, 3, 50), (33, 256, 256, 70, 2)])
+def test_dc_exclude_option(n, N, K, T, F):
+    """MWAX_OPT_DC_EXCLUDE: 1 (default) removes the DC fine channel from the centre output channel and
+    re-scales it, 0 leaves the step out; both against the oracle's weight tables, with a DC offset on every input so that
+    the two differ by far more than the tolerance."""
+    spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[synth.Tone(0, 12.0, 0)], seed=600 + n + N)
+    volt = synth.gauss_voltages(spec)
+    ref_on = oracle.fx(volt, N, K, T, F)
+    ref_off = oracle.fx(volt, N, K, T, F, oracle.AVG_KEEP_DC)
+    got_on = _run_fx(volt, n, N, K, T, F)[0]
+    got_off = _run_fx(volt, n, N, K, T, F, options=[(corr.MWAX_OPT_DC_EXCLUDE, 0)])[0]
+    back_on = _run_fx(volt, n, N, K, T, F, options=[(corr.MWAX_OPT_DC_EXCLUDE, 0), (corr.MWAX_OPT_DC_EXCLUDE, 1)])[0]
+    assert _norm_err(got_on, ref_on, n) <= TOL
+    assert _norm_err(got_off, ref_off, n) <= TOL
+    assert np.array_equal(back_on, got_on)
+    c0 = (K // F) // 2
+    assert got_off[c0, 0].real > 3.0 * got_on[c0, 0].real, "with the exclusion off the DC offset must show in the centre channel"
+
+
 def test_fx_additivity_over_dumps_and_batch_layout():
     """process_batch with a row pitch longer than one integration: dump d uses samples [dTN, (d+1)TN) of every
     row; an integration over 2T equals the sum of the two integrations over T."""
@@ -223,6 +270,13 @@ def test_fx_full_size_configs_sampled(name):
     for d in range(D):
         ref = oracle.fx(volt, N, K, T, F, dump=d, sel=np.array(SEL))
         assert _norm_err(_gather_sel(got[d], SEL), ref, len(SEL)) <= TOL
+    # a seeded-random selection as well (SEL sits on tile edges; a wrong store INSIDE a 256 x 256 tile would pass it):
+    # 16 inputs on dump 0, and 64 inputs = 2080 baselines on every channel of dump 1
+    rng = np.random.default_rng(20260 + len(name) + N)
+    for d, m in ((0, 16), (1, 64)):
+        rsel = np.sort(rng.choice(n, size=m, replace=False))
+        ref = oracle.fx(volt, N, K, T, F, dump=d, sel=rsel)
+        assert _norm_err(_gather_sel(got[d], rsel), ref, m) <= TOL
     ii = np.arange(n)
     autos = got[..., ii * (ii + 1) // 2 + ii]
     assert np.all(autos.imag == 0.0) and np.all(autos.real >= 0.0)
@@ -255,6 +309,93 @@ def test_fx_config5_shape_two_coarse_channels_sampled():
             assert _norm_err(_gather_sel(got[c, d], sel), ref, len(sel)) <= TOL
 
 
+def test_fx_config5_full_batch_last_coarse_channel():
+    """BASELINE.json configs[4] WHOLE: 8 coarse channels x 1024 inputs x 0.5 s through one process_batch call (10.5 GB in,
+    8.6 GB out: byte offsets beyond 4 GiB on both sides); the oracle checks coarse channel 7, dump 1 and coarse channel 0,
+    dump 0 on a 10-input selection.  Coarse channels 1..6 reuse channel 0's samples (generation time), 7 has its own."""
+    cfg = synth.CONFIGS["C5"]
+    n, N, K, T, F, D = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg, cfg.n_dumps
+    NCO = 8
+    dev = torch.empty((NCO, n, cfg.samples_per_input, 2), dtype=torch.int8, device="cuda")
+    host = torch.empty((n, cfg.samples_per_input, 2), dtype=torch.int8).pin_memory()
+    synth.gauss_voltages(cfg.spec(coarse=0), out=host.numpy())
+    first = host.numpy().copy()
+    for c in range(NCO - 1):
+        dev[c].copy_(host)
+    synth.gauss_voltages(cfg.spec(coarse=7), out=host.numpy())
+    dev[NCO - 1].copy_(host)
+    h = corr.MwaxCorr(n, N, K, T, F)
+    out = h.new_output(n_dumps=D, n_coarse=NCO)
+    assert dev.numel() > 2 ** 32 and out.numel() * 4 > 2 ** 32
+    h.process_batch(dev, out, D, NCO)
+    torch.cuda.synchronize()
+    sel = [0, 1, 63, 64, 500, 511, 512, 767, 1000, 1023]
+    for (c, d, volt) in ((NCO - 1, 1, host.numpy()), (0, 0, first)):
+        got = _complex(out[c, d].cpu().numpy())
+        ref = oracle.fx(volt, N, K, T, F, dump=d, sel=np.array(sel))
+        assert _norm_err(_gather_sel(got, sel), ref, len(sel)) <= TOL
+    # channels 1..6 saw channel 0's samples: same bits
+    assert torch.equal(out[3].view(torch.int32), out[0].view(torch.int32))
+    h.destroy()
+
+
+def test_host_buffer_entry_full_config3_against_oracle():
+    """The e2e leg of bench.py: mwax_corr_process_host at BASELINE.json configs[2]'s full size (two dumps, the last one
+    leaving in four channel ranges) against the oracle on SEL, and bit-identical to the device entry."""
+    cfg = synth.CONFIGS["C3"]
+    n, N, K, T, F, D = cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg, cfg.n_dumps
+    hv = torch.empty((1, n, cfg.samples_per_input, 2), dtype=torch.int8).pin_memory()
+    synth.gauss_voltages(cfg.spec(), out=hv.numpy()[0])
+    h = corr.MwaxCorr(n, N, K, T, F)
+    hout = torch.full((1, D, K // F, n * (n + 1) // 2, 2), float("nan"), dtype=torch.float32).pin_memory()
+    h.process_host(hv, hout, D, 1)
+    dev = h.new_output(n_dumps=D)
+    h.process_batch(hv.cuda(), dev, D)
+    torch.cuda.synchronize()
+    assert torch.equal(hout.view(torch.int32), dev.cpu().view(torch.int32))
+    got = _complex(hout.numpy()[0])
+    for d in range(D):
+        ref = oracle.fx(hv.numpy()[0], N, K, T, F, dump=d, sel=np.array(SEL))
+        assert _norm_err(_gather_sel(got[d], SEL), ref, len(SEL)) <= TOL
+    # streaming accumulation has no host entry (the sum would live in the staging buffer): refused, nothing enqueued
+    h.set_accumulate(True)
+    with pytest.raises(corr.MwaxError):
+        h.process_host(hv, hout, D, 1)
+    h.destroy()
+
+
+def test_two_live_handles_of_different_lengths_alternate():
+    """Several handles may be alive at once (include/mwax_corr.h).  Kernel attributes are per device, not per handle: a
+    generic-kernel plan with a large shared tile (N = 2048), one with a small tile (N = 100) and a specialised one
+    (N = 6400, given a misaligned buffer so that it falls back to the generic kernel with ITS tile) keep working in any order."""
+    shapes = [(12, 2048, 2048, 3, 1), (12, 100, 100, 6, 5), (8, 6400, 6400, 2, 50)]
+    hs, vs, refs = [], [], []
+    for k, (n, N, K, T, F) in enumerate(shapes):
+        volt = synth.gauss_voltages(synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[], seed=50 + k))
+        refs.append(oracle.fx(volt, N, K, T, F))
+        hs.append(corr.MwaxCorr(n, N, K, T, F))
+        if N == 6400:
+            buf = torch.empty(volt.size + 2, dtype=torch.int8, device="cuda")
+            v = buf[2:].view(volt.shape)       # 2 bytes off 16-byte alignment: scalar-load generic kernel
+            v.copy_(torch.from_numpy(volt))
+        else:
+            v = torch.from_numpy(volt).cuda()
+        vs.append(v)
+    for order in ((0, 1, 2), (2, 0, 1), (1, 2, 0), (0, 2, 1)):
+        for k in order:
+            n, N, K, T, F = shapes[k]
+            out = hs[k].new_output()
+            out.fill_(float("nan"))
+            if N == 6400:
+                hs[k].process_batch(vs[k][None], out, 1)
+            else:
+                hs[k].process(vs[k], out[0, 0])
+            torch.cuda.synchronize()
+            assert _norm_err(_complex(out.cpu().numpy()[0, 0]), refs[k], n) <= TOL
+    for h in hs:
+        h.destroy()
+
+
 @pytest.mark.parametrize("n,N,K,T,F,D,NCO", [
     (32, 128, 128, 20, 2, 2, 1),
     (70, 320, 300, 6, 3, 1, 2),      # two coarse channels through the reused staging; 100 output channels in 4 uneven ranges
@@ -285,6 +426,8 @@ def test_host_buffer_entry_matches_device_entry(n, N, K, T, F, D, NCO):
     (12, 100, 100, 7, 5),       # generic Stockham kernel
     (10, 6400, 6400, 3, 50),    # the paper's mode: three-pass cluster kernel, ragged group
     (6, 6400, 5000, 2, 50),     # keep < fft at N = 6400
+    (300, 128, 128, 20, 1),     # several pair tiles and ten 32-input F groups
+    (40, 6400, 6400, 2, 50),    # five 8-input work items of the N = 6400 kernel
 ])
 def test_delay_phase_correction_elementwise(n, N, K, T, F):
     rng = np.random.default_rng(100 + n + N)
@@ -324,6 +467,7 @@ def test_delay_phase_correction_elementwise(n, N, K, T, F):
     (12, 100, 100, 7, 5, 1),       # generic Stockham kernel, BLOCK mode
     (10, 6400, 6400, 3, 50, 0),    # the paper's mode: the three-pass kernel leaves its 2-bit weight codes for the table
     (6, 6400, 5000, 2, 50, 0),     # keep < fft at N = 6400
+    (300, 256, 256, 10, 2, 0),     # several pair tiles and ten 32-input F groups
 ])
 def test_channel_gains_elementwise(n, N, K, T, F, mode):
     rng = np.random.default_rng(300 + n + N)
@@ -547,17 +691,14 @@ def test_caller_owned_workspace_gives_the_same_result():
     (200, 256, 256, 70, 2, 1),     # config-5 shape cut down, several pair tiles, the whole band as one run
     (8, 6400, 6400, 64, 50, 7),    # the paper's mode: 49 interior taps per channel
 ])
-def test_shared_edge_schedule_matches_oracle(monkeypatch, n, N, K, T, F, runs):
+def test_shared_edge_schedule_matches_oracle(n, N, K, T, F, runs):
     """Even F, centre-symmetric averaging: the pair kernel's shared-edge schedule (each half-weight edge channel contracted
     once per run of adjacent output channels) against the oracle, and against the plain schedule."""
     spec = synth.GaussSpec(n, N * T, N, sigma=16.0, rho=0.2, tones=[synth.Tone(3, 6.0, 1)], seed=4000 + n + N + runs)
     volt = synth.gauss_voltages(spec)
     ref = oracle.fx(volt, N, K, T, F, 0)
-    monkeypatch.setenv("MWAX_X_EDGE", "1")
-    monkeypatch.setenv("MWAX_X_EDGE_RUNS", str(runs))
-    got = _run_fx(volt, n, N, K, T, F, 0)[0]
-    monkeypatch.setenv("MWAX_X_EDGE", "0")
-    plain = _run_fx(volt, n, N, K, T, F, 0)[0]
+    got = _run_fx(volt, n, N, K, T, F, 0, options=[(corr.MWAX_OPT_X_EDGE_RUNS, runs)])[0]
+    plain = _run_fx(volt, n, N, K, T, F, 0, options=[(corr.MWAX_OPT_X_EDGE_RUNS, 0)])[0]
     assert not np.isnan(got.view(np.float64)).any()
     assert _norm_err(got, ref, n) <= TOL
     assert _norm_err(plain, ref, n) <= TOL
@@ -566,15 +707,15 @@ def test_shared_edge_schedule_matches_oracle(monkeypatch, n, N, K, T, F, runs):
     assert np.all(got[:, ii * (ii + 1) // 2 + ii].imag == 0.0)
 
 
-def test_shared_edge_schedule_with_streaming_accumulation(monkeypatch):
+def test_shared_edge_schedule_with_streaming_accumulation():
     """MWAX_OPT_ACCUMULATE under the shared-edge schedule: two blocks added equal one integration."""
     n, N, K, T, F = 16, 64, 64, 64, 2
     spec = synth.GaussSpec(n, N * 2 * T, N, sigma=16.0, rho=0.2, tones=[], seed=4242)
     volt = synth.gauss_voltages(spec)
     ref = oracle.fx(volt, N, K, 2 * T, F, 0)
-    monkeypatch.setenv("MWAX_X_EDGE", "1")
-    monkeypatch.setenv("MWAX_X_EDGE_RUNS", "3")
     h = corr.MwaxCorr(n, N, K, T, F)
+    h.set_option(corr.MWAX_OPT_X_EDGE_RUNS, 3)
+    assert h.x_edge_runs() == 3
     v = torch.from_numpy(volt).cuda()
     out = h.new_output()
     out.fill_(float("nan"))
@@ -589,9 +730,9 @@ def test_shared_edge_schedule_with_streaming_accumulation(monkeypatch):
 
 @pytest.mark.parametrize("n,N,K,T,F", [
     (512, 128, 128, 600, 1),     # C3 kernels (pow2 F, pair X, every SM busy for several waves)
-    (70, 6400, 6400, 6, 50),     # C4 kernels (three-pass F with the cluster row exchange)
+    (70, 6400, 6400, 6, 50),     # C4 kernels (three-pass F, sub-item 0 parked in tensor memory)
     (300, 256, 256, 96, 2),      # C5 kernels (shared-edge X schedule where the chooser picks it)
-    (40, 320, 300, 9, 3),        # generic F kernel, single-CTA tiles with ragged edges
+    (40, 320, 300, 9, 3),        # generic F kernel, one ragged pair tile
 ])
 def test_repeated_runs_are_bit_identical_and_do_not_depend_on_earlier_calls(n, N, K, T, F):
     """The path has a fixed summation order (no atomics): the same input must give the same BITS on every launch, into
