@@ -451,6 +451,9 @@ int mwax_oracle_xcorr_i8(int n_sel, const int *sel, int n_inputs, int n_chan, in
 #ifdef _OPENMP
 #include <omp.h>
 int mwax_oracle_threads(void) { return omp_get_max_threads(); }
+/* timing infrastructure only (bench.py's single-thread run of config C1); no arithmetic depends on it */
+void mwax_oracle_set_threads(int n) { if (n >= 1) omp_set_num_threads(n); }
 #else
 int mwax_oracle_threads(void) { return 1; }
+void mwax_oracle_set_threads(int n) { (void)n; }
 #endif

@@ -60,6 +60,8 @@ def _load():
                                               ctypes.c_int, dp, dp]
         lib.mwax_oracle_xcorr_i8.argtypes = [ctypes.c_int, ip, ctypes.c_int, ctypes.c_int, ctypes.c_int, i8p, i32p]
         lib.mwax_oracle_threads.argtypes = []
+        lib.mwax_oracle_set_threads.argtypes = [ctypes.c_int]
+        lib.mwax_oracle_set_threads.restype = None
         _lib = lib
     return _lib
 
@@ -80,6 +82,11 @@ def _sel(sel, n_inputs):
 
 def threads() -> int:
     return int(_load().mwax_oracle_threads())
+
+
+def set_threads(n: int) -> None:
+    """OpenMP threads of the following calls (timing infrastructure: bench.py's single-thread run of config C1)."""
+    _load().mwax_oracle_set_threads(int(n))
 
 
 def dft_naive(x: np.ndarray) -> np.ndarray:

@@ -102,6 +102,19 @@ __device__ __forceinline__ float2 apply_delay_gain(float2 v, DelayGain gn, int u
     return make_float2(fmaf(v.x, cs, -v.y * sn), fmaf(v.x, sn, v.y * cs));
 }
 
+// The gain along a run of bins u0, u0 + du, u0 + 2 du, ... is a geometric sequence: the register kernels take the sine
+// and cosine once per run (delay_gain_at) and once per (input, frame) for the ratio (delay_gain_at with pt = 0) and walk
+// the run with one complex multiply per bin.  Runs are 8 bins long (16 at most), so the walk adds a few 1e-7 of error;
+// round 1's sine + cosine per bin kept the quarter-rate XU pipe busier than the FFT kept the FMA pipe.
+__device__ __forceinline__ float2 delay_gain_at(float pt, float st, int u)
+{
+    float tr = fmaf((float)u, st, pt);
+    tr -= rintf(tr);                                                 // [-0.5, 0.5] turns, exact
+    float sn, cs;
+    __sincosf(tr * 6.283185307179586f, &sn, &cs);
+    return make_float2(cs, sn);
+}
+
 // y_k = sum_j x_j w_R^{jk}, forward (w_R = exp(-2 pi i / R))
 template <int R>
 __device__ __forceinline__ void butterfly(float2 (&x)[R]);

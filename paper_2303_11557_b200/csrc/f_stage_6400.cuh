@@ -230,6 +230,7 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
             DelayGain gn = {0.f, 0.f};
             if (DELAY && i_in < P.n_inputs)
                 gn = load_delay_gain(P.delay, P.phase, (long long)i_in * P.d_stride + P.frame0 + t, 1.0f / (float)C::N);
+            const float2 gs = DELAY ? delay_gain_at(0.0f, gn.st, 400) : make_float2(1.0f, 0.0f);
             const int col = grp * C::GI + 2 * g;                     // complex column of this thread's input pair
             const bool col_ok = col < P.pitch2;
             const char *ycol = reinterpret_cast<const char *>(P.Y + (size_t)t * P.y_t_stride + col);
@@ -249,9 +250,15 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
                 fft_dif<16>(z);
                 const uint32_t code = (FULL && SCALE) ? codes[c] : 0u;   // 2 bits per k3: 0 -> 1, 1 -> sqrt(1/2), 2 -> 0
                 if (DELAY) {
+                    // bins u = c + 400 k3 (k3 < 8) and u = c - 3200 + 400 (k3 - 8): two geometric runs of ratio gs
+                    float2 gq = delay_gain_at(gn.pt, gn.st, c);
+                    const float2 gneg = delay_gain_at(gn.pt, gn.st, c - C::N / 2);
 #pragma unroll
-                    for (int k3 = 0; k3 < 16; ++k3)
-                        z[bitrev(k3, 4)] = apply_delay_gain(z[bitrev(k3, 4)], gn, c + 400 * k3 - (k3 < 8 ? 0 : C::N));
+                    for (int k3 = 0; k3 < 16; ++k3) {
+                        if (k3 == 8) gq = gneg;
+                        z[bitrev(k3, 4)] = cmul(z[bitrev(k3, 4)], gq);
+                        if (k3 != 7 && k3 != 15) gq = cmul(gq, gs);
+                    }
                 }
                 if (FULL && SCALE && code != 0u) {                   // rare: 8 + 1 of the 400 tasks at F = 50
 #pragma unroll

@@ -234,6 +234,12 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
         if (DELAY && iok) gn = load_delay_gain(P.delay, P.phase, (long long)i * P.d_stride + P.frame0 + t, 1.0f / (float)N);
 
         // ---- pass 2: this thread's k1 = w*KPT + e; X[k1 + R1 k2] = FFT_R2 over r
+        // DELAY: the gains of the bins u = k1 + R1 k2 (k2 < R2/2) and u = k1 - N/2 + R1 (k2 - R2/2) are two geometric runs of
+        // ratio gs; each run is walked as CH interleaved chains of ratio gs^CH (one dependent chain of complex multiplies in
+        // the store loop of this latency-bound kernel cost more than the sine and cosine per bin it replaced)
+        constexpr int CH = (R2 / 2 >= 4) ? 4 : R2 / 2;
+        const float2 gs = DELAY ? delay_gain_at(0.0f, gn.st, R1) : make_float2(1.0f, 0.0f);
+        const float2 gsc = DELAY ? delay_gain_at(0.0f, gn.st, R1 * CH) : make_float2(1.0f, 0.0f);
 #pragma unroll
         for (int e = 0; e < C::KPT; ++e) {
             const int k1 = w * C::KPT + e;
@@ -241,6 +247,22 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
 #pragma unroll
             for (int r = 0; r < R2; ++r) y[r] = ex_r[(e * R2 + r) * 32];
             fft_dif<R2>(y);
+            if (DELAY) {
+                // gains in place, before the store loop: g[k2] for both runs
+#pragma unroll
+                for (int hrun = 0; hrun < 2; ++hrun) {
+                    float2 gq[CH];
+                    gq[0] = delay_gain_at(gn.pt, gn.st, hrun ? k1 - N / 2 : k1);
+#pragma unroll
+                    for (int j = 1; j < CH; ++j) gq[j] = cmul(gq[j - 1], gs);
+#pragma unroll
+                    for (int q = 0; q < R2 / 2; ++q) {
+                        const int k2 = hrun * (R2 / 2) + q;
+                        y[bitrev(k2, ilog2(R2))] = cmul(y[bitrev(k2, ilog2(R2))], gq[q % CH]);
+                        if (q + CH < R2 / 2) gq[q % CH] = cmul(gq[q % CH], gsc);
+                    }
+                }
+            }
             if (FULL) {
                 // k < N/2  <=>  k2 < R2/2:  p = k + N/2, else p = k - N/2
                 __half2 *yp = ybase + ((size_t)(k1 + N / 2) * P.T + t) * P.pitch2;
@@ -250,7 +272,6 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) {
                         float2 v = y[bitrev(k2, ilog2(R2))];
-                        if (DELAY) v = apply_delay_gain(v, gn, k1 + ((k2 < R2 / 2) ? R1 * k2 : R1 * k2 - N));
                         const int pk = (k2 < R2 / 2) ? (N / 2 + R1 * k2) : (R1 * k2 - N / 2);   // p - k1
                         if (SCALE) {
                             const float f = swp[pk];
@@ -270,7 +291,6 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                     const int p = u + half;                                  // centre order
                     if (p < 0 || p >= P.K) continue;                         // keep the central K channels (L611)
                     float2 v = y[bitrev(k2, ilog2(R2))];
-                    if (DELAY) v = apply_delay_gain(v, gn, u);
                     if (SCALE) {
                         const float f = swt[p];                              // sqrt(w_p): shared edge / DC exclusion
                         v.x *= f;

@@ -75,6 +75,20 @@ def test_int8_bit_exact_elementwise(n, n_chan, n_time):
     h.destroy()
 
 
+@pytest.mark.parametrize("n,n_chan,n_time", [(72, 9, 300), (13, 5, 129), (200, 3, 64)])
+def test_int8_host_buffer_entry_bit_exact(n, n_chan, n_time):
+    """mwax_xcorr_i8_process_host: channel ranges pipelined over three streams (fewer channels than ranges included),
+    rows padded to 16 bytes on the way in when n % 8 != 0."""
+    z = synth.uniform_voltages(n_chan, n_time, n, n_shared=min(64, n), seed=300 + n)
+    h = corr.MwaxXcorrI8(n, n_chan, n_time)
+    hz = torch.from_numpy(z).contiguous().pin_memory()
+    hout = torch.full((n_chan, n * (n + 1) // 2, 2), -7, dtype=torch.int32).pin_memory()
+    for _ in range(2):      # the second call reuses the staging buffers
+        h.process_host(hz, hout)
+    assert np.array_equal(hout.numpy(), oracle.xcorr_i8(z))
+    h.destroy()
+
+
 def test_int8_extreme_values_bit_exact():
     """-128 and +127 everywhere it hurts: accumulator magnitude 2*128^2*T stays exact in int32."""
     n, n_chan, n_time = 24, 2, 4000
