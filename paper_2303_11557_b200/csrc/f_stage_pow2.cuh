@@ -108,7 +108,7 @@ struct FPow2Config {
     static constexpr int VPT = (32 * (N / 8)) / THREADS;   // 16-byte raw vectors per thread per frame
     static_assert(RPT >= 1 && KPT >= 1 && (RPT == 1 || RPT == 2), "unsupported split");
     static_assert(R1 * R2 == N && W * RPT == R2 && W * KPT == R1, "bad factorisation");
-    static_assert(VPT * THREADS == 32 * (N / 8), "raw tile must divide evenly over the threads");
+    static_assert(VPT * THREADS == 32 * (N / 8) && THREADS % 8 == 0, "raw tile must divide evenly over the threads");
     static_assert(R1 % 4 == 0, "twiddle rows are read as 16-byte pairs");
 };
 
@@ -144,8 +144,11 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
     bool rok[C::VPT];
 #pragma unroll
     for (int v = 0; v < C::VPT; ++v) {
+        // a warp covers 4 rows x 8 vectors (128 contiguous bytes of each row): its four 32-bit stores of a stash go to the
+        // words row * ROW_WORDS + 4 c + k = row + 4 c + k (mod 32), all 32 banks once (2 rows x 16 vectors had c and c + 8
+        // collide: 8.7 M conflict wavefronts per C3 launch on the kernel's busiest unit, the L1 data pipe)
         const int idx = threadIdx.x + v * C::THREADS;
-        const int row = idx / VPR, c = idx % VPR;
+        const int row = (idx >> 3) & 31, c = ((idx >> 3) >> 5) * 8 + (idx & 7);
         rok[v] = (i0 + row) < P.n_inputs;
         src[v] = P.volt + 2 * ((long long)(rok[v] ? i0 + row : 0) * P.row_pitch + P.sample0) + 16 * c;
         rdst[v] = raw + row * C::ROW_WORDS + 4 * c;
@@ -229,7 +232,6 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
             }
         }
         __syncthreads();                                              // ex complete; raw(t) no longer needed
-        if (more) stash(q);
         DelayGain gn = {0.f, 0.f};
         if (DELAY && iok) gn = load_delay_gain(P.delay, P.phase, (long long)i * P.d_stride + P.frame0 + t, 1.0f / (float)N);
 
@@ -300,6 +302,10 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                 }
             }
         }
+        // the prefetched bytes of frame t + 1 go into the raw tile as LATE as possible (the tile is free from the first barrier
+        // on): stashed right after pass 1, as in round 1, the store waited for the loads and held 28 % of the kernel's stall
+        // samples (profiles/r2_ncu_full.md); here they have had both passes to arrive
+        if (more) stash(q);
         __syncthreads();                                              // ex consumed; raw(t+1) visible
     }
 }
