@@ -37,7 +37,12 @@ struct FParams {
     int frame0;
     __half2 *Y;              // [K][T][pitch2]
     int pitch2;              // half2 (complex) elements per Y row
-    unsigned y_p_stride, y_t_stride;   // half2 elements between channel positions / between spectra (p3 kernel)
+    unsigned y_p_stride, y_t_stride;   // half2 elements between channel positions / between spectra (N = 6400 kernel)
+    // Register kernels (N = 64 .. 512) only: their two small tables travel in the KERNEL-PARAMETER constant bank, so that the
+    // warp-uniform reads of them are constant-cache loads and not wavefronts of the L1 data pipe, the busiest unit of those
+    // kernels (profiles/r2_ncu_full.md).  twc[r * R1 + k1] = W_N^{r k1} (R1 = 8 for N <= 128, else 16); swc[p] = sw[p].
+    float2 twc[512];
+    float swc[512];
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)

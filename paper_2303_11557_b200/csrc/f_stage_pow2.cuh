@@ -101,10 +101,8 @@ struct FPow2Config {
     static constexpr int KPT = PTS / R2;          // k1 values per thread in pass 2
     static constexpr int ROW_WORDS = N / 2 + 1;   // padded raw row: bank(row, word) = row + word (mod 32)
     static constexpr int RAW_WORDS = 32 * ROW_WORDS;
-    static constexpr int TW_WORDS = 2 * N;        // inter-pass twiddles [r][k1] float2
-    static constexpr int EX_OFF_WORDS = ((RAW_WORDS + TW_WORDS + 3) / 4) * 4;
-    static constexpr int SW_OFF_WORDS = EX_OFF_WORDS + N * 32 * 2;    // per-position factors sqrt(w_p) [K <= N] (SCALE variants)
-    static constexpr int SMEM_BYTES = SW_OFF_WORDS * 4 + N * 4;
+    static constexpr int EX_OFF_WORDS = ((RAW_WORDS + 3) / 4) * 4;
+    static constexpr int SMEM_BYTES = (EX_OFF_WORDS + N * 32 * 2) * 4;   // raw tile + fp32 exchange buffer
     static constexpr int VPT = (32 * (N / 8)) / THREADS;   // 16-byte raw vectors per thread per frame
     static_assert(RPT >= 1 && KPT >= 1 && (RPT == 1 || RPT == 2), "unsupported split");
     static_assert(R1 * R2 == N && W * RPT == R2 && W * KPT == R1, "bad factorisation");
@@ -121,24 +119,15 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
     constexpr int R2 = C::R2;
     extern __shared__ __align__(16) uint32_t fsm[];
     uint32_t *raw = fsm;                                              // [32 rows][ROW_WORDS]
-    float2 *twp = reinterpret_cast<float2 *>(fsm + C::RAW_WORDS + (C::RAW_WORDS & 1));   // [R2][R1] W_N^{r k1}
     float2 *ex = reinterpret_cast<float2 *>(fsm + C::EX_OFF_WORDS);  // [k1][r][lane]
-    float *swt = reinterpret_cast<float *>(fsm + C::SW_OFF_WORDS);   // sqrt(w_p): the channel of a store is warp uniform, so
-                                                                      // these are broadcast reads (was a global load per bin)
+    // inter-pass twiddles W_N^{r k1} and per-position factors sqrt(w_p): constant-bank tables in the kernel parameters (FParams)
 
     const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i0 = blockIdx.x * 32;
     const int t_begin = blockIdx.y * P.frames_per_cta;
     const int t_end = min(P.T, t_begin + P.frames_per_cta);
 
-    // ---- per-CTA setup: twiddle rows, row pointers
-    for (int e = threadIdx.x; e < N; e += C::THREADS) {
-        const int r = e / R1, k1 = e % R1;
-        twp[e] = __ldg(&P.tw[r * k1]);
-    }
-    if (SCALE)
-        for (int e = threadIdx.x; e < P.K; e += C::THREADS) swt[e] = __ldg(&P.sw[e]);
-    constexpr int VPR = N / 8;                                        // 16-byte vectors per row
+    // ---- per-CTA setup: row pointers
     const int8_t *src[C::VPT];
     uint32_t *rdst[C::VPT];
     bool rok[C::VPT];
@@ -187,7 +176,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
     const uint32_t *rrow = raw + lane * C::ROW_WORDS + (C::RPT == 2 ? w : (w >> 1));
     float2 *ex_w = ex + (w * C::RPT) * 32 + lane;                     // + (k1 * R2 + e) * 32
     const float2 *ex_r = ex + (w * C::KPT) * R2 * 32 + lane;          // + (e * R2 + r) * 32
-    const float4 *tw_row = reinterpret_cast<const float4 *>(twp + (w * C::RPT) * R1);
+    const float4 *tw_row = reinterpret_cast<const float4 *>(P.twc + (w * C::RPT) * R1);   // rows r = RPT w + e: warp-uniform
 
     // output addressing: position p of bin k = k1 + R1 k2 is k +- N/2 when K == N
     const int i = i0 + lane;
@@ -269,7 +258,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                 // k < N/2  <=>  k2 < R2/2:  p = k + N/2, else p = k - N/2
                 __half2 *yp = ybase + ((size_t)(k1 + N / 2) * P.T + t) * P.pitch2;
                 __half2 *yn = ybase + ((size_t)k1 * P.T + t) * P.pitch2;
-                const float *swp = swt + k1;
+                const float *swp = P.swc + k1;
                 if (iok) {
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) {
@@ -294,7 +283,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                     if (p < 0 || p >= P.K) continue;                         // keep the central K channels (L611)
                     float2 v = y[bitrev(k2, ilog2(R2))];
                     if (SCALE) {
-                        const float f = swt[p];                              // sqrt(w_p): shared edge / DC exclusion
+                        const float f = P.swc[p];                            // sqrt(w_p): shared edge / DC exclusion
                         v.x *= f;
                         v.y *= f;
                     }

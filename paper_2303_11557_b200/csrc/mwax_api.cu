@@ -303,6 +303,7 @@ struct mwax_corr {
     float2 *d_tw;
     unsigned *d_swcode;
     float *d_sw;
+    std::vector<float> h_sw;            // host copy of sw[] for the register kernels' parameter-bank table
     int *d_tap_start;
     float *d_scale;
     uint8_t *d_ptiles;  // CTA-pair tile list
@@ -403,6 +404,7 @@ static int build_tables(mwax_corr *h)
     h->edge_runs = -1;
     int rc;
     if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
+    h->h_sw = sw;
     if (h->N == 6400 && K == 6400) {
         // the three-pass kernel takes sqrt(w_p) as 2-bit codes, one word per c = k mod 400, field k3 = k / 400
         std::vector<unsigned> code(400, 0u);
@@ -420,6 +422,7 @@ static int build_tables(mwax_corr *h)
         h->chan_scale = 1;
         cudaFree(h->d_sw); h->d_sw = nullptr;
         if ((rc = upload(&h->d_sw, sw)) != MWAX_OK) return rc;
+        h->h_sw = sw;
     }
     if ((rc = upload(&h->d_tap_start, tap)) != MWAX_OK) return rc;
     if ((rc = upload(&h->d_scale, scale)) != MWAX_OK) return rc;
@@ -581,6 +584,14 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
         int rc = launch_f_6400(fp, full, scale, delay, h->sm_count, st);
         if (rc != MWAX_OK) return rc;
     } else if (f_kind) {
+        // the register kernels read their twiddles and per-position factors from the kernel parameters (constant bank)
+        const int R1 = f_kind <= 128 ? 8 : 16, R2 = f_kind / R1;
+        for (int r = 0; r < R2; ++r)
+            for (int k1 = 0; k1 < R1; ++k1) {
+                const double a = 2.0 * M_PI * (double)((r * k1) % f_kind) / (double)f_kind;
+                fp.twc[r * R1 + k1] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
+            }
+        for (int p = 0; p < h->K; ++p) fp.swc[p] = h->h_sw[p];
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
         const int groups = (h->n + 31) / 32;
         long long fpc = ((long long)groups * h->T) / ((long long)h->sm_count * 24);
