@@ -114,7 +114,7 @@ def physical_gpu_index(local_rank: int) -> int:
 # The oracle is timed on a FIXED sample (round 1 sized the sample from a calibration run and the extrapolated rate moved
 # 40 % with the sample length): all inputs, all fine channels, the first ORACLE_SPECTRA spectra of dump 0 — the same
 # sample in the cpu_baseline leg of the default run and in every step of --impl reference.
-ORACLE_SPECTRA = {"C3": 2000, "C4": 3, "C5": 100}
+ORACLE_SPECTRA = {"C3": 800, "C4": 3, "C5": 100}
 
 
 def _oracle_fixed_sample(cfg, wl):

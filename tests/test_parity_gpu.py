@@ -136,6 +136,16 @@ def test_config1_tiny_fx_elementwise():
     ref = oracle.fx(volt, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg)
     got = _run_fx(volt, cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg)[0]
     assert _norm_err(got, ref, cfg.n_inputs) <= TOL
+    # the library counts the kernels it enqueues (bench.py's gpu_launches): one F + one X per integration, one for MWAX_ORDER
+    h = corr.MwaxCorr(cfg.n_inputs, cfg.n_fft, cfg.n_keep, cfg.t_int, cfg.f_avg)
+    assert h.launch_count() == 0
+    out = h.new_output()
+    h.process(torch.from_numpy(volt).cuda(), out[0, 0])
+    assert h.launch_count() == 2
+    h.to_mwax_order(out[0, 0])
+    assert h.launch_count() == 3
+    torch.cuda.synchronize()
+    h.destroy()
     # the tone lands at position 5 + 32 with phase 2 pi (i - j) / 16 (reading Q18)
     p = 37
     n = cfg.n_inputs
