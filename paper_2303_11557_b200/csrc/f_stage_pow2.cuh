@@ -11,7 +11,7 @@
 // X[k1 + R1 k2] = sum_r W_R2^{r k2} (W_N^{r k1} A_r[k1]).
 // int8 -> fp32 promotion happens in registers with the power-of-two F-stage scale folded in.
 //
-// The kernel is instruction-issue bound (ncu: profiles/r1_f128_*.md), so everything that is not butterfly
+// The kernel is co-limited by the issue slots, the L1 data pipe and the FMA pipe (ncu: profiles/r2_ncu_full.md), so everything that is not butterfly
 // arithmetic is hoisted out of the frame loop: row pointers, the swizzle-free padded raw tile (row stride N/2+1
 // words -> bank = row + word), inter-pass twiddles read as broadcast 16-byte shared loads, and store addresses
 // formed as base + k2 * stride with compile-time k2.  The raw bytes of frame t+1 are fetched into registers while
