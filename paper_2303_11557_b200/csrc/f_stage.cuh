@@ -77,6 +77,13 @@ __device__ __forceinline__ float2 csub(float2 a, float2 b)
     asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(b)));
     return unpack2(r);
 }
+// (a.x * f, a.y * f) in one issue slot
+__device__ __forceinline__ float2 scale2(float2 a, float f)
+{
+    unsigned long long r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(pack2(a)), "l"(pack2(make_float2(f, f))));
+    return unpack2(r);
+}
 // (a.x * b.x + c.x, a.y * b.y + c.y)
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c)
 {

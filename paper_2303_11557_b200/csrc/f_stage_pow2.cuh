@@ -13,7 +13,7 @@
 //
 // The kernel is co-limited by the issue slots, the L1 data pipe and the FMA pipe (ncu: profiles/r2_ncu_full.md), so everything that is not butterfly
 // arithmetic is hoisted out of the frame loop: row pointers, the swizzle-free padded raw tile (row stride N/2+1
-// words -> bank = row + word), inter-pass twiddles read as broadcast 16-byte shared loads, and store addresses
+// words -> bank = row + word), inter-pass twiddles and per-position factors read from the kernel-parameter constant bank, and store addresses
 // formed as base + k2 * stride with compile-time k2.  The raw bytes of frame t+1 are fetched into registers while
 // frame t is being transformed.
 #pragma once
@@ -264,11 +264,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                     for (int k2 = 0; k2 < R2; ++k2) {
                         float2 v = y[bitrev(k2, ilog2(R2))];
                         const int pk = (k2 < R2 / 2) ? (N / 2 + R1 * k2) : (R1 * k2 - N / 2);   // p - k1
-                        if (SCALE) {
-                            const float f = swp[pk];
-                            v.x *= f;
-                            v.y *= f;
-                        }
+                        if (SCALE) v = scale2(v, swp[pk]);
                         __half2 *dst = (k2 < R2 / 2) ? yp + (size_t)(unsigned)(R1 * k2) * chan_stride      // one IMAD.WIDE.U32
                                                      : yn + (size_t)(unsigned)(R1 * (k2 - R2 / 2)) * chan_stride;
                         *dst = __floats2half2_rn(v.x, v.y);
@@ -282,11 +278,7 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                     const int p = u + half;                                  // centre order
                     if (p < 0 || p >= P.K) continue;                         // keep the central K channels (L611)
                     float2 v = y[bitrev(k2, ilog2(R2))];
-                    if (SCALE) {
-                        const float f = P.swc[p];                            // sqrt(w_p): shared edge / DC exclusion
-                        v.x *= f;
-                        v.y *= f;
-                    }
+                    if (SCALE) v = scale2(v, P.swc[p]);                      // sqrt(w_p): shared edge / DC exclusion
                     ybase[((size_t)p * P.T + t) * P.pitch2] = __floats2half2_rn(v.x, v.y);
                 }
             }
