@@ -304,6 +304,7 @@ struct mwax_corr {
     unsigned *d_swcode;
     float *d_sw;
     std::vector<float> h_sw;            // host copy of sw[] for the register kernels' parameter-bank table
+    std::vector<float2> h_twc;          // W_N^{r k1} as [r][k1], computed once at create() for the same table
     int *d_tap_start;
     float *d_scale;
     uint8_t *d_ptiles;  // CTA-pair tile list
@@ -497,6 +498,15 @@ mwax_corr_t *mwax_corr_create(int n_inputs, int n_fft, int n_keep, int t_int, in
         tw[m] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
     }
     if ((g_last_error = upload(&h->d_tw, tw)) != MWAX_OK) { mwax_corr_destroy(h); return nullptr; }
+    if (h->f_kind && h->f_kind != 6400) {
+        const int R1 = h->f_kind <= 128 ? 8 : 16, R2 = h->f_kind / R1;
+        h->h_twc.resize((size_t)h->f_kind);
+        for (int r = 0; r < R2; ++r)
+            for (int k1 = 0; k1 < R1; ++k1) {
+                const double a = 2.0 * M_PI * (double)((r * k1) % h->f_kind) / (double)h->f_kind;
+                h->h_twc[(size_t)r * R1 + k1] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
+            }
+    }
     // workspace Y[K][T][pitch] fp16, zeroed once (pad columns stay zero)
     h->y_bytes = (size_t)n_keep * t_int * h->pitch * sizeof(__half);
     if (cudaMalloc(reinterpret_cast<void **>(&h->d_Y), h->y_bytes) != cudaSuccess) {
@@ -585,13 +595,8 @@ static int f_stage_impl(mwax_corr_t *h, const int8_t *d_volt, size_t row_pitch, 
         if (rc != MWAX_OK) return rc;
     } else if (f_kind) {
         // the register kernels read their twiddles and per-position factors from the kernel parameters (constant bank)
-        const int R1 = f_kind <= 128 ? 8 : 16, R2 = f_kind / R1;
-        for (int r = 0; r < R2; ++r)
-            for (int k1 = 0; k1 < R1; ++k1) {
-                const double a = 2.0 * M_PI * (double)((r * k1) % f_kind) / (double)f_kind;
-                fp.twc[r * R1 + k1] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
-            }
-        for (int p = 0; p < h->K; ++p) fp.swc[p] = h->h_sw[p];
+        std::memcpy(fp.twc, h->h_twc.data(), h->h_twc.size() * sizeof(float2));
+        std::memcpy(fp.swc, h->h_sw.data(), (size_t)h->K * sizeof(float));
         // frames per CTA: enough CTAs for ~8 waves of 3 resident CTAs per SM, at most 32 frames each
         const int groups = (h->n + 31) / 32;
         long long fpc = ((long long)groups * h->T) / ((long long)h->sm_count * 24);
