@@ -185,6 +185,16 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
     const unsigned chan_stride = (unsigned)P.T * (unsigned)P.pitch2;  // half2 elements between positions (< 2^32: checked at create)
     __half2 *ybase = P.Y + i;
 
+    // store addressing: one pointer chain per k1 where a thread has ONE k1 (N <= 128: -1.4 % at N = 128); with two (N >= 256)
+    // the extra live pointers spill under the two-CTA register budget and cost 4.6 %, so those keep (p, t) addressing
+    constexpr bool CHAIN = (C::KPT == 1);
+    unsigned cs_reg;                                                  // chan_stride in a general register for the whole loop (the
+    asm volatile("mov.u32 %0, %1;" : "=r"(cs_reg) : "r"(chan_stride));   // compiler re-materialised it from the constant bank per store)
+    const unsigned row_bytes = (unsigned)P.pitch2 * 4u;
+    char *yq[C::KPT];
+#pragma unroll
+    for (int e = 0; e < C::KPT; ++e)
+        yq[e] = reinterpret_cast<char *>(ybase + ((size_t)(w * C::KPT + e) * P.T + t_begin) * P.pitch2);
     for (int t = t_begin; t < t_end; ++t) {
         const bool more = (t + 1) < t_end;
         if (more) fetch(t + 1, q);                                    // in flight during both passes
@@ -254,7 +264,24 @@ __global__ void __launch_bounds__(FPow2Config<N, R1, PTS>::THREADS, FPow2Config<
                     }
                 }
             }
-            if (FULL) {
+            if (FULL && CHAIN) {
+                // K == N: the thread's R2 bins k1 + R1 k2 land on the positions p = k1 + R1 j, j = (k2 + R2/2) mod R2: ONE chain of
+                // R2 rows, R1 channel positions apart, from a per-thread pointer that moves one spectrum per frame.  (Forming
+                // every address from (p, t) cost ~60 integer instructions per frame, an eighth of the kernel's issue slots.)
+                const float *swp = P.swc + k1;
+                char *dst = yq[e];
+                if (iok) {
+#pragma unroll
+                    for (int jj = 0; jj < R2; ++jj) {
+                        const int k2 = (jj + R2 / 2) % R2;
+                        float2 v = y[bitrev(k2, ilog2(R2))];
+                        if (SCALE) v = scale2(v, swp[R1 * jj]);
+                        *reinterpret_cast<__half2 *>(dst) = __floats2half2_rn(v.x, v.y);
+                        dst += (unsigned long long)cs_reg * (unsigned)(R1 * 4);       // one IMAD.WIDE.U32
+                    }
+                }
+                yq[e] += row_bytes;
+            } else if (FULL) {
                 // k < N/2  <=>  k2 < R2/2:  p = k + N/2, else p = k - N/2
                 __half2 *yp = ybase + ((size_t)(k1 + N / 2) * P.T + t) * P.pitch2;
                 __half2 *yn = ybase + ((size_t)k1 * P.T + t) * P.pitch2;
