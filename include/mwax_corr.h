@@ -48,7 +48,8 @@ enum {
     MWAX_ERR_UNSUPPORTED = -3, /* n_fft not 2^a*5^b or > 6400, n_keep > n_fft, f_avg !| n_keep  */
     MWAX_ERR_NOMEM = -4,       /* host or device allocation failed                              */
     MWAX_ERR_CUDA = -5,        /* a CUDA runtime/driver call failed; see mwax_corr_last_cuda_error */
-    MWAX_ERR_ARCH = -6         /* no CUDA device, or the current device is not sm_100           */
+    MWAX_ERR_ARCH = -6,        /* no CUDA device, or the current device is not sm_100           */
+    MWAX_ERR_TOO_LARGE = -7    /* mwax_corr_process_static: spectra exceed the static workspace */
 };
 
 /* options for mwax_corr_set_option */
@@ -186,6 +187,31 @@ int mwax_corr_x_edge_runs(mwax_corr_t *h);
 long long mwax_corr_launch_count(const mwax_corr_t *h);
 int mwax_corr_last_cuda_error(const mwax_corr_t *h);
 int mwax_corr_destroy(mwax_corr_t *h); /* NULL is a no-op returning MWAX_OK */
+
+/* ------------------------------------------------------------------------------------------------------
+ * Allocation-free entry (no handle): one integration through the same F and X kernels as
+ * mwax_corr_create(n_inputs, n_fft, n_fft, t_int, f_avg) + mwax_corr_process with default options (every bin kept,
+ * centre-symmetric averaging, DC excluded), for callers that may not call cudaMalloc: code under CUDA-graph
+ * capture, tight serving loops, harnesses that forbid allocation.  The call makes NO cudaMalloc / cudaFree / host-to-
+ * device copy: the fp16 spectra Y[n_fft][t_int][pitch] (pitch = 2 n_inputs rounded up to 64) that the path keeps
+ * between its two kernels live in a static device array inside the library, MWAX_STATIC_Y_BYTES = 32 MiB (plus 64 KiB
+ * of tables filled on the device), which every GPU that loads the library holds until the process exits.
+ *   d_volt in : int8 [n_inputs][t_int * n_fft][re,im], contiguous rows, 16-byte aligned (else MWAX_ERR_INVALID_ARG)
+ *   d_vis  out: float [n_fft / f_avg][n(n+1)/2][re,im]  (caller-owned, as for mwax_corr_process)
+ *   n_fft  in {64, 128, 256, 512} (the kernels whose tables travel in the kernel parameters; else MWAX_ERR_UNSUPPORTED),
+ *   f_avg divides n_fft, n_inputs <= 8128.
+ * Limit: n_fft * t_int * pitch * 2 bytes <= mwax_corr_static_workspace_max() = MWAX_STATIC_Y_BYTES, otherwise
+ * MWAX_ERR_TOO_LARGE is returned and nothing is enqueued (e.g. 128 inputs x 128 channels x 512 spectra = 32 MiB fits).
+ * The array is SHARED by every call on a device and keeps the last call's contents (the call clears what it needs
+ * zero): two calls that overlap on the GPU (different streams or threads without an ordering between them) race.
+ * Work is enqueued on `stream` (3-4 operations: optional clear, table kernel, F kernel, X kernel); the call is
+ * asynchronous like mwax_corr_process.  The first call on a device sets kernel attributes and looks the array's
+ * address up (cudaGetSymbolAddress); make it once outside a graph capture.
+ * ---------------------------------------------------------------------------------------------------- */
+#define MWAX_STATIC_Y_BYTES (32u * 1024u * 1024u)
+#define MWAX_STATIC_TABLE_BYTES (64u * 1024u)
+size_t mwax_corr_static_workspace_max(void);
+int mwax_corr_process_static(const int8_t *d_volt, float *d_vis, int n_inputs, int n_fft, int t_int, int f_avg, void *stream);
 
 /* ------------------------------------------------------------------------------------------------------
  * X-only integer path (BASELINE.json configs[1]): the X-stage contraction on pre-channelised int8

@@ -95,6 +95,9 @@ def lib() -> ctypes.CDLL:
         L.mwax_xcorr_i8_process.argtypes = [vp, vp, vp, vp]
         L.mwax_xcorr_i8_process_host.argtypes = [vp, vp, vp, vp]
         L.mwax_xcorr_i8_destroy.argtypes = [vp]
+        L.mwax_corr_static_workspace_max.restype = sz
+        L.mwax_corr_static_workspace_max.argtypes = []
+        L.mwax_corr_process_static.argtypes = [vp, vp, i32, i32, i32, i32, vp]
         L.mwax_corr_strerror.restype = ctypes.c_char_p
         L.mwax_corr_strerror.argtypes = [i32]
         L.mwax_corr_version.restype = ctypes.c_char_p
@@ -272,6 +275,24 @@ class MwaxCorr:
             self.destroy()
         except Exception:
             pass
+
+
+def static_workspace_max() -> int:
+    """Bytes of fp16 spectra (n_fft * t_int * roundup(2 n_inputs, 64) * 2) that process_static() can hold."""
+    return int(lib().mwax_corr_static_workspace_max())
+
+
+def process_static(volt: torch.Tensor, vis: torch.Tensor, n_inputs: int, n_fft: int, t_int: int, f_avg: int, stream=None):
+    """mwax_corr_process_static: one integration without a handle and without any device allocation inside the library
+    (its scratch is a static device array; calls that overlap on the GPU race).  volt int8 cuda [n][T*N][2]; vis float32
+    cuda [N/F][n(n+1)/2][2] (written).  Raises MwaxError (MWAX_ERR_TOO_LARGE) beyond static_workspace_max()."""
+    assert volt.is_cuda and volt.dtype == torch.int8 and volt.is_contiguous()
+    assert vis.is_cuda and vis.dtype == torch.float32 and vis.is_contiguous()
+    assert volt.numel() == n_inputs * t_int * n_fft * 2
+    assert f_avg >= 1 and vis.numel() == (n_fft // f_avg) * (n_inputs * (n_inputs + 1) // 2) * 2
+    _check(lib().mwax_corr_process_static(volt.data_ptr(), vis.data_ptr(), n_inputs, n_fft, t_int, f_avg, _stream_ptr(stream)),
+           "mwax_corr_process_static")
+    return vis
 
 
 class MwaxXcorrI8:

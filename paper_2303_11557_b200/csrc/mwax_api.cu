@@ -448,6 +448,7 @@ const char *mwax_corr_strerror(int code)
         case MWAX_ERR_NOMEM: return "out of memory";
         case MWAX_ERR_CUDA: return "CUDA error";
         case MWAX_ERR_ARCH: return "no sm_100 CUDA device";
+        case MWAX_ERR_TOO_LARGE: return "spectra exceed the static workspace (MWAX_STATIC_Y_BYTES, see mwax_corr_static_workspace_max)";
         default: return "unknown error";
     }
 }
@@ -1011,6 +1012,161 @@ int mwax_xcorr_i8_destroy(mwax_xcorr_t *h)
     }
     delete h;
     return MWAX_OK;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ allocation-free entry
+// mwax_corr_process_static (include/mwax_corr.h): the whole F -> X pass of mwax_corr_process for callers that may not
+// call cudaMalloc (CUDA-graph capture, tight serving loops, harnesses that forbid it).  The fp16 spectra Y that the F
+// kernel writes and the X kernel contracts — the one piece of scratch memory on the path — live in this file-scope
+// array instead of a cudaMalloc'ed workspace, followed by the X kernel's three small tables, which a one-block kernel
+// fills on the device from the call's arguments (no host-to-device copy either).  Every GPU that loads the library holds
+// the array until the process exits; every call on a device shares it, so calls that overlap on the GPU race.
+// In HOST code the array's name is only a stand-in: the device address comes from cudaGetSymbolAddress, once per device.
+static __device__ __align__(256) unsigned char g_static_ws[MWAX_STATIC_Y_BYTES + MWAX_STATIC_TABLE_BYTES];
+
+namespace {
+
+struct StaticTables {          // offsets into the table region that follows the Y scratch
+    static constexpr size_t TILES = 0;              // uint8 [n_tiles][4], n_tiles <= 2080 (n <= 8128)
+    static constexpr size_t TAP = 16 * 1024;        // int   [C], C <= 512
+    static constexpr size_t SCALE = 32 * 1024;      // float [C]
+};
+static_assert(MWAX_STATIC_TABLE_BYTES >= 48 * 1024 && MWAX_STATIC_Y_BYTES % 256 == 0, "table region layout");
+
+// the tables build_tables() uploads, for the default options (centre-symmetric averaging, DC excluded): PAPER.md L290-298
+__global__ void static_tables_kernel(uint8_t *tiles, int *tap, float *scale, int n_tiles, int C, int K, int F, float sc, float sc_c0)
+{
+    for (int e = threadIdx.x; e < n_tiles; e += blockDim.x) {
+        int mi = 0;
+        while ((mi + 1) * (mi + 2) / 2 <= e) ++mi;                   // e = mi (mi + 1) / 2 + nj, nj <= mi
+        const int nj = e - mi * (mi + 1) / 2;
+        tiles[4 * e + 0] = (uint8_t)mi; tiles[4 * e + 1] = (uint8_t)nj; tiles[4 * e + 2] = 0; tiles[4 * e + 3] = 0;
+    }
+    const int c0 = C / 2, half = K / 2, dmax = (F % 2) ? (F - 1) / 2 : F / 2;
+    for (int c = threadIdx.x; c < C; c += blockDim.x) {
+        const int u0 = (c - c0) * F - dmax;
+        tap[c] = (F == 1) ? c : ((u0 + half) % K + K) % K;
+        scale[c] = (F > 1 && c == c0) ? sc_c0 : sc;
+    }
+}
+
+struct StaticDevice {
+    unsigned char *ws;         // device address of g_static_ws on this device
+    DevicePlan dp;
+    int sm_count;
+};
+
+// once per device, with that device current: kernel attributes (prepare_device) and the array's device address
+int static_device(StaticDevice *out)
+{
+    static std::mutex mu;
+    static std::map<int, StaticDevice> done;
+    int sm = 0, dev = 0, rc;
+    if ((rc = check_device(&sm, &dev)) != MWAX_OK) return rc;
+    std::lock_guard<std::mutex> lock(mu);
+    auto it = done.find(dev);
+    if (it != done.end()) { *out = it->second; return MWAX_OK; }
+    StaticDevice sd;
+    sd.sm_count = sm;
+    if ((rc = prepare_device(dev, sm, &sd.dp)) != MWAX_OK) return rc;
+    void *p = nullptr;
+    if (cudaGetSymbolAddress(&p, g_static_ws) != cudaSuccess || !p) { cudaGetLastError(); return MWAX_ERR_CUDA; }
+    sd.ws = static_cast<unsigned char *>(p);
+    done[dev] = sd;
+    *out = sd;
+    return MWAX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t mwax_corr_static_workspace_max(void) { return (size_t)MWAX_STATIC_Y_BYTES; }
+
+int mwax_corr_process_static(const int8_t *d_volt, float *d_vis, int n_inputs, int n_fft, int t_int, int f_avg, void *stream)
+{
+    if (!d_volt || !d_vis) return MWAX_ERR_NULL;
+    if (n_inputs < 1 || n_fft < 1 || t_int < 1 || f_avg < 1) return MWAX_ERR_INVALID_ARG;
+    // the register kernels keep their tables in the kernel parameters: no device table, hence these four lengths only
+    if ((n_fft != 64 && n_fft != 128 && n_fft != 256 && n_fft != 512) || n_fft % f_avg != 0 || n_inputs > 8128) return MWAX_ERR_UNSUPPORTED;
+    if (reinterpret_cast<uintptr_t>(d_volt) & 15u) return MWAX_ERR_INVALID_ARG;     // 16-byte loads (no scalar-load kernel here)
+    const int N = n_fft, K = n_fft, T = t_int, F = f_avg, C = K / F, n = n_inputs;
+    const int pitch = ((2 * n + 63) / 64) * 64;                                      // fp16 elements per Y row, as create()
+    const unsigned long long y_bytes = (unsigned long long)K * (unsigned long long)T * (unsigned long long)pitch * sizeof(__half);
+    if (y_bytes > (unsigned long long)MWAX_STATIC_Y_BYTES) return MWAX_ERR_TOO_LARGE;
+    StaticDevice sd;
+    int rc = static_device(&sd);
+    if (rc != MWAX_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    __half *Y = reinterpret_cast<__half *>(sd.ws);
+    unsigned char *tab = sd.ws + MWAX_STATIC_Y_BYTES;
+    uint8_t *d_tiles = tab + StaticTables::TILES;
+    int *d_tap = reinterpret_cast<int *>(tab + StaticTables::TAP);
+    float *d_scale = reinterpret_cast<float *>(tab + StaticTables::SCALE);
+
+    // the array keeps the last call's contents.  Every column of an input < n is rewritten by the F kernel below; the pad
+    // columns (2n not a multiple of 64) must read as zero and may hold another shape's spectra: cleared here
+    if (pitch != 2 * n && cudaMemsetAsync(Y, 0, (size_t)y_bytes, st) != cudaSuccess) { cudaGetLastError(); return MWAX_ERR_CUDA; }
+
+    // averaging geometry of build_tables(), default options
+    const int lg = (int)std::ceil(std::log2((double)N) / 2.0);
+    const double s = std::ldexp(1.0, -lg);
+    const float sc = (float)(1.0 / (s * s * F));
+    const float sc_c0 = F > 1 ? (float)((1.0 / (s * s * F)) * (double)F / (double)(F - 1)) : sc;
+    const int n_tiles = ((n + 127) / 128) * ((n + 127) / 128 + 1) / 2;
+    const int n_taps = (F == 1) ? 1 : 2 * ((F % 2) ? (F - 1) / 2 : F / 2) + 1;
+    static_tables_kernel<<<1, 256, 0, st>>>(d_tiles, d_tap, d_scale, n_tiles, C, K, F, sc, sc_c0);
+
+    // F stage: f_stage_impl()'s register-kernel launch with Y = the static array
+    mwax::FParams fp;
+    std::memset(&fp, 0, sizeof(fp));
+    fp.volt = d_volt; fp.row_pitch = (long long)T * N; fp.sample0 = 0;
+    fp.n_inputs = n; fp.N = N; fp.K = K; fp.T = T; fp.G = 32; fp.vec_ok = 1;
+    fp.in_scale = (float)s; fp.chan_scale = F > 1 ? 1 : 0;
+    fp.Y = reinterpret_cast<__half2 *>(Y); fp.pitch2 = pitch / 2;
+    fp.y_p_stride = (unsigned)T * (unsigned)(pitch / 2); fp.y_t_stride = (unsigned)(pitch / 2);
+    const int R1 = N <= 128 ? 8 : 16, R2 = N / R1;
+    for (int r = 0; r < R2; ++r)
+        for (int k1 = 0; k1 < R1; ++k1) {
+            const double a = 2.0 * M_PI * (double)((r * k1) % N) / (double)N;
+            fp.twc[r * R1 + k1] = make_float2((float)std::cos(a), (float)(-std::sin(a)));
+        }
+    for (int p = 0; p < K; ++p) {
+        const int u = p - K / 2;
+        fp.swc[p] = (F > 1 && F % 2 == 0 && (((u - F / 2) % F) + F) % F == 0) ? (float)std::sqrt(0.5) : 1.0f;
+    }
+    if (F > 1) fp.swc[K / 2] = 0.0f;                                                 // DC excluded (L290-294)
+    const int groups = (n + 31) / 32;
+    long long fpc = ((long long)groups * T) / ((long long)sd.sm_count * 24);
+    fpc = fpc < 1 ? 1 : (fpc > 32 ? 32 : fpc);
+    fp.frames_per_cta = (int)fpc;
+    const int chunks = (T + (int)fpc - 1) / (int)fpc;
+    const bool scale = fp.chan_scale != 0;
+    switch (N) {
+        case 64: launch_f_pow2<64, 8, 16>(fp, true, scale, false, groups, chunks, st); break;
+        case 128: launch_f_pow2<128, 8, 16>(fp, true, scale, false, groups, chunks, st); break;
+        case 256: launch_f_pow2<256, 16, 32>(fp, true, scale, false, groups, chunks, st); break;
+        default: launch_f_pow2<512, 16, 32>(fp, true, scale, false, groups, chunks, st); break;
+    }
+    if (cudaGetLastError() != cudaSuccess) return MWAX_ERR_CUDA;
+
+    // X stage: x_stage_range()'s launch over all channels; the tensor maps are encoded on the host (no device memory)
+    CUtensorMap tmap, tmap_flat;
+    if ((rc = encode_z_map(&tmap, false, Y, (uint64_t)pitch, (uint64_t)pitch * 2, (uint64_t)T, (uint64_t)K, 64)) != MWAX_OK) return rc;
+    if ((rc = encode_z_map(&tmap_flat, false, Y, (uint64_t)pitch, (uint64_t)pitch * 2, (uint64_t)T * K, 1, 64)) != MWAX_OK) return rc;
+    mwax::XParams xp;
+    xp.n_inputs = n; xp.T = T; xp.K = K; xp.n_out = C; xp.n_tiles = n_tiles;
+    xp.tiles = d_tiles; xp.tap_start = d_tap; xp.n_taps = n_taps; xp.scale = d_scale;
+    xp.out_chan_stride = (long long)n * (n + 1) / 2;
+    xp.out = d_vis;
+    xp.accumulate = 0;
+    xp.edge_runs = (n_taps == F + 1) ? choose_edge_runs(C, F, T, n_tiles, sd.dp.pairs_f16_edge, -1) : 0;
+    rc = xp.edge_runs > 0 ? launch_x_pair<false, true>(tmap, tmap_flat, xp, sd.dp.pairs_f16_edge, st)
+                          : launch_x_pair<false>(tmap, tmap_flat, xp, sd.dp.pairs_f16, st);
+    if (rc != MWAX_OK) cudaGetLastError();
+    return rc;
 }
 
 }  // extern "C"

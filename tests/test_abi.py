@@ -53,6 +53,26 @@ def test_argument_validation_is_synchronous_and_needs_no_gpu():
     assert L.mwax_corr_process(None, None, None, None) == -1
 
 
+def test_static_entry_validates_sizes_without_a_gpu_and_calls_no_allocator():
+    """mwax_corr_process_static: the size limit is checked before any device is touched, and the function's source has no
+    allocating call (the scratch is a static device array whose address comes from cudaGetSymbolAddress)."""
+    import ctypes
+    L = corr.lib()
+    buf = ctypes.create_string_buffer(64)
+    a = (ctypes.addressof(buf) + 15) & ~15
+    assert L.mwax_corr_static_workspace_max() == 32 * 1024 * 1024
+    assert L.mwax_corr_process_static(a, a, 128, 128, 513, 1, None) == -7            # 128 x 513 x 256 x 2 B > 32 MiB
+    assert b"static workspace" in L.mwax_corr_strerror(-7)
+    assert L.mwax_corr_process_static(a, a, 128, 100, 4, 1, None) == -3              # no register kernel for N = 100
+    assert L.mwax_corr_process_static(a + 1, a, 128, 128, 4, 1, None) == -2          # misaligned voltages
+    assert L.mwax_corr_process_static(None, a, 128, 128, 4, 1, None) == -1
+    src = open(os.path.join(ROOT, "paper_2303_11557_b200", "csrc", "mwax_api.cu")).read()
+    body = src[src.index("static __device__ __align__(256)"):]
+    assert "cudaGetSymbolAddress" in body
+    for banned in ("cudaMalloc", "cudaFree", "cudaMemcpy", "upload("):
+        assert banned not in body, banned
+
+
 def test_library_reads_no_environment_variables():
     """Every knob is an argument or a set_option key (include/mwax_corr.h): no getenv in the product sources."""
     csrc = os.path.join(ROOT, "paper_2303_11557_b200", "csrc")
