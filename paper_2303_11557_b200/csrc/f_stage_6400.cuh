@@ -13,11 +13,13 @@
 // sectors into read-modify-write DRAM traffic (profiles/r1_ncu_full.md), so round 1 exchanged rows between the two
 // CTAs of a cluster (15 % of the kernel on the push + wait, 21 % on a separate store phase).  Here a work item is
 // (frame t, group of EIGHT adjacent inputs), done as two sub-items of four inputs, thread g <-> input 2 g + s:
-//   sub-item s = 0: pass 3 rounds its results to fp16 and PARKS them in tensor memory (tcgen05.st, thread-private
-//                   lanes: TMEM is 256 KB of otherwise idle on-chip storage in this kernel; 102 KB are used);
-//   sub-item s = 1: pass 3 reads the parked words back (tcgen05.ld) and stores {input 2 g, input 2 g + 1} = 8 bytes
-//                   per thread, four adjacent lanes = one whole 32-byte sector, straight from registers while the
-//                   other warps are still computing.
+//   pass 3 of BOTH sub-items rounds its results to fp16 and PARKS them in tensor memory (tcgen05.st, thread-private
+//   lanes: TMEM is 256 KB of otherwise idle on-chip storage in this kernel; 204 KB are used), sub-item 1 next to sub-item 0;
+//   the item then leaves during passes 1 and 2 of the NEXT item's first sub-item: at twelve points of those passes every
+//   thread reads four bins of both sub-items back (tcgen05.ld) and stores {input 2 g, input 2 g + 1} = 8 bytes per bin,
+//   four adjacent lanes = one whole 32-byte sector.  Issued in one burst at the end of pass 3 the 6400 scattered sectors of
+//   an item held 30 % of the kernel (2.38 ms, 1.66 ms with the stores removed: the LSU takes a cycle per 128-byte line an
+//   instruction touches, eight per STG.64 here, and 20 warps x 16 stores queued at once); spread out they cost half of that.
 // Every global LOAD of the steady state is the raw voltage itself, one sub-item ahead (see fetch()).
 #pragma once
 #include <cuda_fp16.h>
@@ -78,8 +80,9 @@ struct F6400 {
     static constexpr int T2_OFF = T1_OFF + 400;                      // s W_320^{n3 k2} [n3][21], 336 float2
     static constexpr int CODE_OFF = T2_OFF + 336;                    // 400 x uint32 weight codes (as 200 float2)
     static constexpr int SMEM_BYTES = (CODE_OFF + 200) * 8;          // 225,728
-    static constexpr int TMEM_COLS = 256;                            // 5 warps per lane quadrant x 48 columns
-    static constexpr int PARK_STRIDE = 48;                           // columns per warp: 3 rounds x 16 words
+    static constexpr int TMEM_COLS = 512;                            // 5 warps per lane quadrant x 96 columns
+    static constexpr int PARK_STRIDE = 96;                           // columns per warp: 2 sub-items x 3 rounds x 16 words
+    static constexpr int PARK_SUB = 48;                              // column offset of sub-item 1's words
     static_assert(S2 % 2 == 1 && S1 % 16 == 5 && SG % 16 == 4 && T1_OFF % 2 == 0, "bank-conflict-free strides, 16-byte aligned tables");
     static_assert(5 * PARK_STRIDE <= TMEM_COLS, "parked rows of the five warps of a lane quadrant");
 };
@@ -93,14 +96,12 @@ __device__ __forceinline__ void tmem_st_32x32b_x16(uint32_t taddr, const uint32_
           "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
         : "memory");
 }
-__device__ __forceinline__ void tmem_ld_32x32b_x16(uint32_t taddr, uint32_t (&r)[16])
+__device__ __forceinline__ void tmem_ld_32x32b_x4(uint32_t taddr, uint32_t (&r)[4])
 {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-          "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
-        : "r"(taddr)
-        : "memory");
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(taddr)
+                 : "memory");
 }
 // streaming 4-byte load that does not allocate an L1 line (the shared tile leaves this kernel almost no L1)
 __device__ __forceinline__ uint32_t ld_stream_u32(const void *p)
@@ -142,9 +143,7 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
     const uint32_t park = *reinterpret_cast<volatile uint32_t *>(&tmem_slot) + ((uint32_t)((warp & 3) * 32) << 16) +
                           (uint32_t)((warp >> 2) * C::PARK_STRIDE);
 
-    // pass 3 (and the stores): thread = (input g of 4, task index j of 160): four adjacent lanes = four inputs of one row
-    const int g = threadIdx.x & 3, j = threadIdx.x >> 2;             // j in [0,160)
-    float2 *eg = esm + g * C::SG;
+    float2 *eg = esm + (threadIdx.x & 3) * C::SG;
     // passes 1 and 2 (and the voltage loads): warp = (input gw, five groups v of four middle-index values), lane = (a, lo):
     // the 32 lanes of a load instruction read 128 CONTIGUOUS bytes of one input, one L2 request instead of the four
     // 32-byte ones of (4 inputs x 8 pairs) warps: 400 instead of 1600 read requests per sub-item (measured: -3.5 %)
@@ -179,6 +178,32 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
     const int sub0 = 2 * (int)blockIdx.x, sub_step = 2 * (int)gridDim.x;
     fetch(sub0);
 
+    // Deferred stores.  Pass 3 of BOTH sub-items parks its fp16 rows in tensor memory; the 6400 sectors of item i leave
+    // during passes 1 and 2 of the next item's first sub-item, four stores per thread at each of twelve points spread over
+    // those passes (point pt: round r = pt / 4, bins k3 = 4 (pt % 4) ...+3).  Issued in one burst at the end of pass 3 they
+    // cost 30 % of the kernel: the SM sends one 32-byte sector per clock to L2, 20 warps x 16 stores x 8 sectors queued at
+    // once, and every warp sat on the full queue (profiles/r2_f6400.md).
+    const unsigned cs_bytes = chan_stride * 4u;                      // bytes between channel positions (< 2^32: checked by the plan)
+    const int g = threadIdx.x & 3, j = threadIdx.x >> 2;             // pass 3: thread = (input g of 4, task index j of 160)
+    const char *yold = nullptr;                                      // column base of the parked item's rows (this thread's input pair)
+    auto store_point = [&](int pt) {
+        const int r = pt >> 2, k3b = (pt & 3) * 4;
+        const int c = j + 160 * r;
+        if (c >= 400) return;                                        // warp-uniform (r = 2: warps 0..9)
+        uint32_t pa[4], pb[4];
+        tmem_ld_32x32b_x4(park + (uint32_t)(16 * r + k3b), pa);
+        tmem_ld_32x32b_x4(park + (uint32_t)(C::PARK_SUB + 16 * r + k3b), pb);
+        ptx::tmem_ld_wait();
+        // rows p = u + K/2 of the signed bins u = c + 400 k3 (k3 < 8), c - 3200 + 400 (k3 - 8) (k3 >= 8): centre order (L290), keep (L611)
+        const int p0 = c + half + 400 * (k3b & 7) - (k3b < 8 ? 0 : C::N / 2);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int p = p0 + 400 * q;
+            if (FULL || (p >= 0 && p < P.K))
+                *reinterpret_cast<uint2 *>(const_cast<char *>(yold) + (size_t)(unsigned)p * cs_bytes) = make_uint2(pa[q], pb[q]);
+        }
+    };
+
     for (int sub_a = sub0; sub_a < n_sub; sub_a += sub_step) {
 #pragma unroll 1
         for (int s = 0; s < 2; ++s) {
@@ -188,8 +213,10 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
 
             // ---- pass 1: tasks (n2 = hi, n3 = 2 lo + rep): 20-point FFT over n1 of x[320 n1 + 16 n2 + n3], then W_400^{n2 k1}
             float2 x[5][4];
+            const bool drain = (s == 0) && (yold != nullptr);        // this sub-item's passes 1-2 carry the previous item's stores
 #pragma unroll
             for (int rep = 0; rep < 2; ++rep) {
+                if (drain) store_point(3 * rep);
 #pragma unroll
                 for (int a = 0; a < 5; ++a)
 #pragma unroll
@@ -205,10 +232,12 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
                         x[a][b] = cadd(m, make_float2(-8388736.0f, -8388736.0f));
                     }
                 fft20(x);
+                if (drain) store_point(3 * rep + 1);
                 const float4 *trow = reinterpret_cast<const float4 *>(t1 + hi * 20);   // four rows per warp, 160 bytes apart: one wavefront
                 float2 *ew = egw + hi * C::S2 + 2 * lo + rep;
 #pragma unroll
                 for (int k1 = 0; k1 < 20; k1 += 2) {
+                    if (k1 == 10 && drain) store_point(3 * rep + 2);
                     const float4 tw = trow[k1 / 2];
                     const float2 v0 = x[k1 % 5][k1 / 5], v1 = x[(k1 + 1) % 5][(k1 + 1) / 5];
                     ew[k1 * C::S1] = (k1 == 0) ? v0 : cmul(v0, make_float2(tw.x, tw.y));
@@ -228,9 +257,14 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
                 for (int a = 0; a < 5; ++a)
 #pragma unroll
                     for (int b = 0; b < 4; ++b) x[a][b] = e[(4 * a + b) * C::S2];
+                if (drain) store_point(6 + 3 * rep);
                 fft20(x);
+                if (drain) store_point(7 + 3 * rep);
 #pragma unroll
-                for (int k2 = 0; k2 < 20; ++k2) e[k2 * C::S2] = cmul(x[k2 % 5][k2 / 5], cmul(trow[k2], cw));
+                for (int k2 = 0; k2 < 20; ++k2) {
+                    if (k2 == 10 && drain) store_point(8 + 3 * rep);
+                    e[k2 * C::S2] = cmul(x[k2 % 5][k2 / 5], cmul(trow[k2], cw));
+                }
             }
             __syncthreads();
 
@@ -244,13 +278,8 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
             if (DELAY && i_in < P.n_inputs)
                 gn = load_delay_gain(P.delay, P.phase, (long long)i_in * P.d_stride + P.frame0 + t, 1.0f / (float)C::N);
             const float2 gs = DELAY ? delay_gain_at(0.0f, gn.st, 400) : make_float2(1.0f, 0.0f);
-            const int col = grp * C::GI + 2 * g;                     // complex column of this thread's input pair
-            const bool col_ok = col < P.pitch2;
-            const char *ycol = reinterpret_cast<const char *>(P.Y + (size_t)t * P.y_t_stride + col);
-            const unsigned cs_bytes = chan_stride * 4u;              // bytes between channel positions (< 2^32: checked by the plan)
-
-            // ---- pass 3: tasks c = k1 + 20 k2 = j + 160 r: 16-point FFT over n3 -> bins k = c + 400 k3, rounded to fp16;
-            // s = 0: parked in TMEM; s = 1: stored together with the parked partner
+            // ---- pass 3: tasks c = k1 + 20 k2 = j + 160 r: 16-point FFT over n3 -> bins k = c + 400 k3, rounded to fp16 and
+            // parked in TMEM (sub-item 1 next to sub-item 0: together they are the 8 bytes this thread stores per bin)
 #pragma unroll 1
             for (int r = 0; r < 3; ++r) {
                 const int c = j + 160 * r;
@@ -296,29 +325,19 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
                     const __half2 h2 = __floats2half2_rn(v.x, v.y);
                     hv[k3] = *reinterpret_cast<const uint32_t *>(&h2);
                 }
-                if (s == 0) {
-                    tmem_st_32x32b_x16(park + (uint32_t)(16 * r), hv);
-                } else {
-                    uint32_t pk[16];
-                    tmem_ld_32x32b_x16(park + (uint32_t)(16 * r), pk);
-                    ptx::tmem_ld_wait();
-                    if (col_ok) {
-                        // rows p = u + K/2 of the signed bins u = c + 400 k3 (k3 < 8), c - 3200 + 400 (k3 - 8) (k3 >= 8): centre
-                        // order (L290), keep (L611).  Two row bases, then one widening multiply-add per store.
-                        const char *ya = ycol + (long long)(c + half) * (long long)cs_bytes;
-                        const char *yb = ycol + (long long)(c + half - C::N / 2) * (long long)cs_bytes;
-#pragma unroll
-                        for (int k3 = 0; k3 < 16; ++k3) {
-                            const int p = c + 400 * k3 - (k3 < 8 ? 0 : C::N) + half;
-                            char *dst = const_cast<char *>(k3 < 8 ? ya : yb) + (size_t)(unsigned)(400 * (k3 & 7)) * cs_bytes;
-                            if (FULL || (p >= 0 && p < P.K)) *reinterpret_cast<uint2 *>(dst) = make_uint2(pk[k3], hv[k3]);
-                        }
-                    }
-                }
+                tmem_st_32x32b_x16(park + (uint32_t)(C::PARK_SUB * s + 16 * r), hv);
             }
-            if (s == 0) tmem_st_wait();
+            tmem_st_wait();
+            if (s != 0) {                                            // the item is complete in TMEM: its rows leave during the next passes 1-2
+                const int col = grp * C::GI + 2 * g;                 // complex column of this thread's input pair (< pitch2: 8 | 32)
+                yold = reinterpret_cast<const char *>(P.Y + (size_t)t * P.y_t_stride + col);
+            }
             __syncthreads();                                         // pass 3 has read E: the next pass 1 may overwrite it
         }
+    }
+    if (yold != nullptr) {                                           // the CTA's last item
+#pragma unroll 1
+        for (int pt = 0; pt < 12; ++pt) store_point(pt);
     }
     ptx::tc_fence_before();
     __syncthreads();
