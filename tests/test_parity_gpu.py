@@ -175,7 +175,10 @@ def test_config1_tiny_fx_elementwise():
     (10, 6400, 6400, 3, 50, 0),    # inputs not a multiple of the 4-input group of the 80 x 80 kernel
     (6, 6400, 5000, 2, 50, 0),     # keep < fft at N = 6400 (oversampled coarse channel, L611)
     (7, 6400, 6400, 2, 50, 1),     # BLOCK mode at N = 6400
-    (16, 6400, 6400, 60, 50, 0),   # 120 work items over 74 persistent clusters: the exchange buffer is re-used between items
+    (16, 6400, 6400, 60, 50, 0),   # 120 work items on 148 CTAs: one item each, every row leaves in the kernel's final flush
+    (48, 6400, 6400, 37, 50, 0),   # 222 work items on 148 CTAs: half the CTAs store one item during the next item's passes
+                                   # 1-2 and flush the second, the others flush their only one
+    (48, 6400, 4000, 37, 50, 0),   # the same with keep < fft: the deferred stores carry the row-range predicate
 ])
 def test_fx_elementwise_shapes(n, N, K, T, F, mode):
     tones = [synth.Tone(min(3, K // 2 - 1), 6.0, 1)] if K > 8 else []
