@@ -77,7 +77,7 @@ struct F6400 {
     static constexpr int S1 = 20 * S2 + 1, SG = 20 * S1;             // float2 strides of k1 and of the input
     static constexpr int E_F2 = G * SG;
     static constexpr int T1_OFF = E_F2;                              // W_400^{n2 k1} [n2][k1], 400 float2
-    static constexpr int T2_OFF = T1_OFF + 400;                      // s W_320^{n3 k2} [n3][21], 336 float2
+    static constexpr int T2_OFF = T1_OFF + 400;                      // s W_320^{n3 k2}: row pair (n3 = 2 lo, 2 lo + 1) at 42 lo, the odd row 22 in: 336 float2
     static constexpr int CODE_OFF = T2_OFF + 336;                    // 400 x uint32 weight codes (as 200 float2)
     static constexpr int SMEM_BYTES = (CODE_OFF + 200) * 8;          // 225,728
     static constexpr int TMEM_COLS = 512;                            // 5 warps per lane quadrant x 96 columns
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
     }
     for (int e = threadIdx.x; e < 320; e += C::THREADS) {
         const float2 w = __ldg(&P.tw[(20 * (e / 20) * (e % 20)) % C::N]);
-        t2[(e / 20) * 21 + e % 20] = make_float2(w.x * P.in_scale, w.y * P.in_scale);
+        t2[(e / 40) * 42 + 22 * ((e / 20) & 1) + e % 20] = make_float2(w.x * P.in_scale, w.y * P.in_scale);
     }
     const int warp = threadIdx.x >> 5;
     if (warp == 0) {
@@ -251,7 +251,7 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
             for (int rep = 0; rep < 2; ++rep) {
                 const int n3 = 2 * lo + rep;
                 float2 *e = egw + hi * C::S1 + n3;
-                const float2 *trow = t2 + n3 * 21;
+                const float4 *trow = reinterpret_cast<const float4 *>(t2 + lo * 42 + 22 * rep);   // (k2, k2 + 1) pairs: 16-byte loads
                 const float2 cw = rep ? cw1 : cw0;
 #pragma unroll
                 for (int a = 0; a < 5; ++a)
@@ -261,9 +261,11 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
                 fft20(x);
                 if (drain) store_point(7 + 3 * rep);
 #pragma unroll
-                for (int k2 = 0; k2 < 20; ++k2) {
+                for (int k2 = 0; k2 < 20; k2 += 2) {
                     if (k2 == 10 && drain) store_point(8 + 3 * rep);
-                    e[k2 * C::S2] = cmul(x[k2 % 5][k2 / 5], cmul(trow[k2], cw));
+                    const float4 tw = trow[k2 / 2];
+                    e[k2 * C::S2] = cmul(x[k2 % 5][k2 / 5], cmul(make_float2(tw.x, tw.y), cw));
+                    e[(k2 + 1) * C::S2] = cmul(x[(k2 + 1) % 5][(k2 + 1) / 5], cmul(make_float2(tw.z, tw.w), cw));
                 }
             }
             __syncthreads();
