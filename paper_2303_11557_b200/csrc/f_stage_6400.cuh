@@ -139,7 +139,7 @@ __global__ void __launch_bounds__(F6400::THREADS, 1) f_stage_6400_kernel(const F
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
-    // this thread's parking place: its own lane of the warp's quadrant, 48 columns per warp of the quadrant
+    // this thread's parking place: its own lane of the warp's quadrant, 96 columns per warp of the quadrant (two sub-items x 48)
     const uint32_t park = *reinterpret_cast<volatile uint32_t *>(&tmem_slot) + ((uint32_t)((warp & 3) * 32) << 16) +
                           (uint32_t)((warp >> 2) * C::PARK_STRIDE);
 

@@ -757,7 +757,7 @@ def test_shared_edge_schedule_with_streaming_accumulation():
 
 @pytest.mark.parametrize("n,N,K,T,F", [
     (512, 128, 128, 600, 1),     # C3 kernels (pow2 F, pair X, every SM busy for several waves)
-    (70, 6400, 6400, 6, 50),     # C4 kernels (three-pass F, sub-item 0 parked in tensor memory)
+    (70, 6400, 6400, 6, 50),     # C4 kernels (three-pass F, both sub-items parked in tensor memory, stores deferred)
     (300, 256, 256, 96, 2),      # C5 kernels (shared-edge X schedule where the chooser picks it)
     (40, 320, 300, 9, 3),        # generic F kernel, one ragged pair tile
 ])
